@@ -1,0 +1,150 @@
+/*
+ * lvsa.h — C ABI of the B200-native LVSA block-sparse attention forward.
+ *
+ * The operation is the one PAPER.md section 2 defines (arxiv/paper_2605_31057):
+ *   Attn(q_{t,i}) = sum_{tau in A(t)} sum_p softmax_{(tau,p)}( q_{t,i} . k_{tau,p} / sqrt(d) ) v_{tau,p}
+ *                                                                        (Eq. 2)
+ *   A(t) = G^s  u  [w_lo(t), w_hi(t)]                                     (Def. 2)
+ *   G^s  = { (s mod T_per + i T_per) mod T : i < ceil(T/T_per) }          (Eq. 3)
+ *   T_per = ceil( T / (C - (2W+1)) )
+ *   (w_lo, w_hi) = Algorithm 1 applied to the adaptive window of PAPER.md:68
+ *
+ * Token layout (reading R12): N = T*P tokens, token n = t*P + p.
+ * Everything runs on ONE GPU (sm_100a).  There is no CPU fallback: without a usable CUDA
+ * device every call below that touches the device returns LVSA_ECUDA / NULL.
+ * No exception crosses this boundary; the only global state is a thread-local error string.
+ */
+#ifndef LVSA_H_
+#define LVSA_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct lvsa_index lvsa_index_t; /* opaque; owns its device and host buffers */
+
+typedef enum {
+    LVSA_OK = 0,
+    LVSA_EINVAL = 1,       /* bad argument (sizes <= 0, W < 0, a < -1, step < 0, NULL, T*P >= 2^31 ...) */
+    LVSA_EUNSUPPORTED = 2, /* legal but not built: head dim / tile / dtype outside {64/64, 128/128} */
+    LVSA_ECUDA = 3,        /* CUDA runtime or driver failure; lvsa_last_error() has the string */
+    LVSA_ENOMEM = 4
+} lvsa_status_t;
+
+#define LVSA_ANCHORS_ALL_TILES (-1) /* anchors value selecting the all-tiles (dense, Eq. 1) path */
+
+enum { LVSA_TILE_FULL = 0, LVSA_TILE_PARTIAL = 1 };            /* values of flags[]            */
+enum { LVSA_TIE_LO = 0, LVSA_TIE_HI = 1 };                     /* Algorithm 1 line 5 tie-break */
+enum { LVSA_DTYPE_BF16 = 0, LVSA_DTYPE_FP32 = 1 };             /* element type of q,k,v,out    */
+enum { LVSA_KERNEL_AUTO = 0, LVSA_KERNEL_SIMT = 1, LVSA_KERNEL_TCGEN05 = 2 };
+
+/* Parameters of lvsa_build_block_index_ex.  Zero means "default" where a default is named. */
+typedef struct lvsa_params {
+    int32_t T;          /* latent frames, >= 1                                                  */
+    int32_t P;          /* tokens per frame, >= 1; T*P < 2^31                                    */
+    int32_t H;          /* heads, >= 1                                                           */
+    int32_t d;          /* head dim: 64 or 128                                                   */
+    int32_t B;          /* batch, default 1                                                      */
+    int32_t window;     /* W >= 0                                                  */
+    int32_t anchors;    /* a = C-(2W+1) >= 0; a >= T: every frame is an anchor;
+                           a == 0: no anchors; LVSA_ANCHORS_ALL_TILES: dense                    */
+    int32_t step;       /* denoising step s >= 0 (Eq. 3)                                        */
+    int32_t layer;      /* >= 0; recorded, does not change the pattern (reading R4)   */
+    int32_t tile_q;     /* default: 128 when d = 128, 64 when d = 64; must equal tile_k         */
+    int32_t tile_k;
+    int32_t tie_break;  /* LVSA_TIE_LO (default) or LVSA_TIE_HI                                 */
+    int32_t dtype;      /* LVSA_DTYPE_BF16 (default, tensor-core kernel) or LVSA_DTYPE_FP32
+                           (SIMT kernel only)                                                   */
+    int32_t kernel;     /* LVSA_KERNEL_AUTO: tcgen05 for bf16, SIMT for fp32                    */
+    float softmax_scale;/* default 1/sqrt(d) (Eq. 1)                                            */
+} lvsa_params_t;
+
+typedef struct lvsa_index_info {
+    int32_t T, P, H, d, B;
+    int32_t window, anchors, step, layer;
+    int32_t tile_q, tile_k;
+    int32_t nq, nk;          /* ceil(N/tile_q), ceil(N/tile_k)                                  */
+    int32_t T_per;           /* 0 when there are no anchors                                     */
+    int32_t phase;           /* s mod T_per                                                     */
+    int32_t n_global;        /* |G^s|                                                           */
+    int32_t words;           /* uint32 words per A(t) bitset = ceil(T/32)                       */
+    int32_t dtype, kernel;
+    int64_t N;               /* T*P                                                             */
+    int64_t nnz;             /* kept (q tile, kv tile) pairs                                    */
+    int64_t n_partial;       /* of which PARTIAL                                                */
+    int64_t n_items;         /* work items of the attention kernel (q-tile groups)              */
+    int64_t n_item_tiles;    /* kv-tile visits over all items (>= nnz / rows-per-item ratio)    */
+} lvsa_index_info_t;
+
+/*
+ * lvsa_build_block_index — steps a1..a5 of the hot path on the GPU (Alg. 1
+ * :74-89, Eq. 3 :97, Def. 2 :49; tile mapping per DESIGN.md reading R14).
+ * Builds, for denoising step `step`, the per-frame attended sets A(t) and the CSR of kept
+ * kv tiles per q tile (tile = 128 tokens for d = 128, 64 for d = 64; tiles start at token 0):
+ *   indptr[nq+1], indices[nnz] ascending within a q tile, flags[nnz] in {FULL, PARTIAL}.
+ * A kv tile is kept iff some (valid query row, valid key column) pair is allowed; it is PARTIAL
+ * iff some (valid row, column of the tile) pair is not (frame not attended, or column >= N).
+ * All arithmetic is integer and runs in CUDA kernels on the current device's default stream;
+ * the call synchronises once to learn nnz.  Returns NULL on error (lvsa_last_error()).
+ * The handle is owned by the library; free it with lvsa_index_destroy.  It is immutable and
+ * may be used by any number of lvsa_attn_fwd calls.
+ */
+lvsa_index_t *lvsa_build_block_index(int T, int P, int H, int d, int window, int anchors,
+                                     int step, int layer);
+
+/* Same with every knob; `stream` is the cudaStream_t the builder kernels run on (NULL = default). */
+lvsa_status_t lvsa_build_block_index_ex(const lvsa_params_t *params, void *stream,
+                                        lvsa_index_t **out);
+
+/*
+ * lvsa_attn_fwd — step a6/a7: Eq. 2 over the kept tiles, exactly (element-level masking on
+ * PARTIAL tiles).
+ *   q, k, v : DEVICE pointers, [B, N, H, d] contiguous (d fastest), bf16 (or fp32 when the index
+ *             was built with LVSA_DTYPE_FP32); 16-byte aligned.  Read-only.
+ *   out     : DEVICE pointer, same shape and dtype as q.  Every element is written.
+ *   lse     : DEVICE pointer, fp32 [B, H, N], lse = ln sum_{kept} exp(q.k/sqrt d) (natural log),
+ *             or NULL.
+ *   stream  : cudaStream_t of the caller (NULL = default stream).
+ * The call only enqueues work on `stream` and returns; it never synchronises and allocates
+ * nothing.  Caller owns all five buffers; the library keeps no reference after the kernels ran.
+ * bf16 inputs: products and sums accumulate in fp32, softmax statistics in fp32, P rounded to
+ * bf16 before P.V, bf16 output.
+ */
+lvsa_status_t lvsa_attn_fwd(const void *q, const void *k, const void *v,
+                            const lvsa_index_t *index, void *out, float *lse, void *stream);
+
+/*
+ * lvsa_attn_fwd_host — the same call for HOST buffers (pinned or pageable): copies q, k, v to
+ * device scratch owned by the index (allocated on first use), runs lvsa_attn_fwd on `stream`,
+ * copies out (and lse if not NULL) back, and synchronises `stream` before returning.
+ */
+lvsa_status_t lvsa_attn_fwd_host(const void *q_host, const void *k_host, const void *v_host,
+                                 lvsa_index_t *index, void *out_host, float *lse_host,
+                                 void *stream);
+
+void lvsa_index_destroy(lvsa_index_t *index);
+
+lvsa_status_t lvsa_index_info(const lvsa_index_t *index, lvsa_index_info_t *info);
+
+/* Copies the index to HOST arrays sized from lvsa_index_info (any pointer may be NULL):
+ * indptr[nq+1], indices[nnz], flags[nnz], w_lo[T], w_hi[T], a_bits[T*words] (bit x of row t set
+ * iff x in A(t), little-endian words).  Synchronises. */
+lvsa_status_t lvsa_index_copy_host(const lvsa_index_t *index, int32_t *indptr, int32_t *indices,
+                                   uint8_t *flags, int32_t *w_lo, int32_t *w_hi,
+                                   uint32_t *a_bits);
+
+/* Number of kernels lvsa_attn_fwd enqueues per call for this index (bench.py's gpu_launches). */
+int lvsa_attn_fwd_launches(const lvsa_index_t *index);
+
+/* Last error message of the calling thread ("" if none).  Never NULL. */
+const char *lvsa_last_error(void);
+
+/* Library version / build string (arch, kernel variants compiled in). */
+const char *lvsa_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LVSA_H_ */

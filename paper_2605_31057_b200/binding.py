@@ -1,0 +1,196 @@
+"""Thin ctypes binding over csrc/liblvsa.so (include/lvsa.h).  Argument marshalling only:
+every step of the hot path (index build, attention) runs in the library's CUDA kernels.
+PyTorch is used by callers for device memory and streams; this module only reads
+`tensor.data_ptr()` and the current stream handle.
+
+There is no CPU fallback.  If the library cannot be built or loaded, importing the symbols
+raises; if there is no CUDA device, the library calls return LVSA_ECUDA and this module raises
+LvsaError.  Nothing here imports oracle/.
+"""
+from __future__ import annotations
+
+import ctypes as C
+from dataclasses import dataclass
+
+import numpy as np
+
+from . import build as _build
+
+ALL_TILES = -1
+TILE_FULL, TILE_PARTIAL = 0, 1
+TIE_LO, TIE_HI = 0, 1
+DTYPE_BF16, DTYPE_FP32 = 0, 1
+KERNEL_AUTO, KERNEL_SIMT, KERNEL_TCGEN05 = 0, 1, 2
+OK, EINVAL, EUNSUPPORTED, ECUDA, ENOMEM = 0, 1, 2, 3, 4
+
+
+class LvsaError(RuntimeError):
+    def __init__(self, status: int, msg: str):
+        super().__init__(f"lvsa status {status}: {msg}")
+        self.status = status
+
+
+class Params(C.Structure):
+    _fields_ = [(n, C.c_int32) for n in
+                ("T", "P", "H", "d", "B", "window", "anchors", "step", "layer", "tile_q", "tile_k",
+                 "tie_break", "dtype", "kernel")] + [("softmax_scale", C.c_float)]
+
+
+class IndexInfo(C.Structure):
+    _fields_ = [(n, C.c_int32) for n in
+                ("T", "P", "H", "d", "B", "window", "anchors", "step", "layer", "tile_q", "tile_k",
+                 "nq", "nk", "T_per", "phase", "n_global", "words", "dtype", "kernel")] + \
+               [(n, C.c_int64) for n in ("N", "nnz", "n_partial", "n_items", "n_item_tiles")]
+
+
+EXPORTS = ("lvsa_build_block_index", "lvsa_build_block_index_ex", "lvsa_attn_fwd",
+           "lvsa_attn_fwd_host", "lvsa_index_destroy", "lvsa_index_info", "lvsa_index_copy_host",
+           "lvsa_attn_fwd_launches", "lvsa_last_error", "lvsa_version")
+
+_lib = None
+
+
+def lib() -> C.CDLL:
+    """Loads (building first if the .so is missing or older than its sources) liblvsa.so."""
+    global _lib
+    if _lib is None:
+        path = _build.build()
+        L = C.CDLL(path)
+        L.lvsa_build_block_index.restype = C.c_void_p
+        L.lvsa_build_block_index.argtypes = [C.c_int] * 8
+        L.lvsa_build_block_index_ex.restype = C.c_int
+        L.lvsa_build_block_index_ex.argtypes = [C.POINTER(Params), C.c_void_p, C.POINTER(C.c_void_p)]
+        L.lvsa_attn_fwd.restype = C.c_int
+        L.lvsa_attn_fwd.argtypes = [C.c_void_p] * 7
+        L.lvsa_attn_fwd_host.restype = C.c_int
+        L.lvsa_attn_fwd_host.argtypes = [C.c_void_p] * 7
+        L.lvsa_index_destroy.restype = None
+        L.lvsa_index_destroy.argtypes = [C.c_void_p]
+        L.lvsa_index_info.restype = C.c_int
+        L.lvsa_index_info.argtypes = [C.c_void_p, C.POINTER(IndexInfo)]
+        L.lvsa_index_copy_host.restype = C.c_int
+        L.lvsa_index_copy_host.argtypes = [C.c_void_p] * 7
+        L.lvsa_attn_fwd_launches.restype = C.c_int
+        L.lvsa_attn_fwd_launches.argtypes = [C.c_void_p]
+        L.lvsa_last_error.restype = C.c_char_p
+        L.lvsa_version.restype = C.c_char_p
+        _lib = L
+    return _lib
+
+
+def lvsa_last_error() -> str:
+    return lib().lvsa_last_error().decode()
+
+
+def lvsa_version() -> str:
+    return lib().lvsa_version().decode()
+
+
+def _check(status: int):
+    if status != OK:
+        raise LvsaError(status, lvsa_last_error())
+
+
+@dataclass
+class HostIndex:
+    indptr: np.ndarray
+    indices: np.ndarray
+    flags: np.ndarray
+    w_lo: np.ndarray
+    w_hi: np.ndarray
+    a_bits: np.ndarray
+
+
+class BlockIndex:
+    """Owns one lvsa_index_t handle."""
+
+    def __init__(self, handle: int):
+        self._h = C.c_void_p(handle)
+
+    @property
+    def handle(self) -> C.c_void_p:
+        if not self._h:
+            raise ValueError("index already destroyed")
+        return self._h
+
+    def info(self) -> IndexInfo:
+        info = IndexInfo()
+        _check(lib().lvsa_index_info(self.handle, C.byref(info)))
+        return info
+
+    def copy_host(self) -> HostIndex:
+        i = self.info()
+        indptr = np.zeros(i.nq + 1, np.int32)
+        indices = np.zeros(i.nnz, np.int32)
+        flags = np.zeros(i.nnz, np.uint8)
+        w_lo = np.zeros(i.T, np.int32)
+        w_hi = np.zeros(i.T, np.int32)
+        a_bits = np.zeros((i.T, i.words), np.uint32)
+        ptr = lambda a: a.ctypes.data_as(C.c_void_p)
+        _check(lib().lvsa_index_copy_host(self.handle, ptr(indptr), ptr(indices), ptr(flags),
+                                          ptr(w_lo), ptr(w_hi), ptr(a_bits)))
+        return HostIndex(indptr, indices, flags, w_lo, w_hi, a_bits)
+
+    def launches(self) -> int:
+        return int(lib().lvsa_attn_fwd_launches(self.handle))
+
+    def destroy(self):
+        if self._h:
+            lib().lvsa_index_destroy(self._h)
+            self._h = C.c_void_p(None)
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+def lvsa_build_block_index(T: int, P: int, H: int, d: int, window: int, anchors: int, step: int,
+                           layer: int) -> BlockIndex:
+    h = lib().lvsa_build_block_index(T, P, H, d, window, anchors, step, layer)
+    if not h:
+        raise LvsaError(-1, lvsa_last_error())
+    return BlockIndex(h)
+
+
+def lvsa_build_block_index_ex(stream: int = 0, **kw) -> BlockIndex:
+    p = Params()
+    for k, v in kw.items():
+        if not hasattr(p, k):
+            raise TypeError(f"unknown lvsa_params_t field {k!r}")
+        setattr(p, k, v)
+    out = C.c_void_p()
+    _check(lib().lvsa_build_block_index_ex(C.byref(p), C.c_void_p(stream), C.byref(out)))
+    return BlockIndex(out.value)
+
+
+def _dev_ptr(t) -> C.c_void_p:
+    if t is None:
+        return C.c_void_p(None)
+    if not t.is_cuda or not t.is_contiguous():
+        raise ValueError("lvsa_attn_fwd takes contiguous CUDA tensors")
+    return C.c_void_p(t.data_ptr())
+
+
+def lvsa_attn_fwd(q, k, v, index: BlockIndex, out, lse=None, stream: int | None = None):
+    """q, k, v, out: CUDA tensors [B, N, H, d]; lse: CUDA fp32 [B, H, N] or None.  Enqueues on
+    `stream` (default: torch's current stream) and returns without synchronising."""
+    if stream is None:
+        import torch
+        stream = torch.cuda.current_stream().cuda_stream
+    _check(lib().lvsa_attn_fwd(_dev_ptr(q), _dev_ptr(k), _dev_ptr(v), index.handle, _dev_ptr(out),
+                               _dev_ptr(lse), C.c_void_p(stream)))
+    return out
+
+
+def lvsa_attn_fwd_host(q, k, v, index: BlockIndex, out, lse=None, stream: int = 0):
+    """Host-buffer variant: q, k, v, out (and lse) are CPU tensors (ideally pinned); copies run
+    inside the call, which returns after the results are back on the host."""
+    hp = lambda t: C.c_void_p(None) if t is None else C.c_void_p(t.data_ptr())
+    for t in (q, k, v, out):
+        if t.is_cuda or not t.is_contiguous():
+            raise ValueError("lvsa_attn_fwd_host takes contiguous CPU tensors")
+    _check(lib().lvsa_attn_fwd_host(hp(q), hp(k), hp(v), index.handle, hp(out), hp(lse),
+                                    C.c_void_p(stream)))
+    return out

@@ -1,0 +1,180 @@
+// C ABI of liblvsa (include/lvsa.h): argument checks, handle lifetime, kernel selection.
+#include <math.h>
+#include <string.h>
+
+#include <new>
+
+#include "lvsa_internal.h"
+
+static thread_local std::string g_last_error;
+
+void lvsa_set_error(const std::string &msg) { g_last_error = msg; }
+
+lvsa_status_t lvsa_cuda_fail(cudaError_t e, const char *what) {
+    g_last_error = std::string(what) + ": " + cudaGetErrorName(e) + " (" + cudaGetErrorString(e) + ")";
+    return LVSA_ECUDA;
+}
+
+static size_t elem_size(const lvsa_index *ix) { return ix->p.dtype == LVSA_DTYPE_FP32 ? 4 : 2; }
+
+static int use_tcgen05(const lvsa_index *ix) {
+    if (ix->p.kernel == LVSA_KERNEL_SIMT) return 0;
+    if (ix->p.kernel == LVSA_KERNEL_TCGEN05) return 1;
+    return ix->p.dtype == LVSA_DTYPE_BF16;
+}
+
+extern "C" {
+
+const char *lvsa_last_error(void) { return g_last_error.c_str(); }
+
+const char *lvsa_version(void) {
+    return "liblvsa 0.1 (sm_100a; kernels: index-builder, attn-simt-fp32, attn-tcgen05-bf16)";
+}
+
+lvsa_status_t lvsa_build_block_index_ex(const lvsa_params_t *params, void *stream, lvsa_index_t **out) {
+    g_last_error.clear();
+    if (out == nullptr || params == nullptr) { lvsa_set_error("NULL params/out"); return LVSA_EINVAL; }
+    *out = nullptr;
+    lvsa_params_t p = *params;
+    if (p.T <= 0 || p.P <= 0 || p.H <= 0 || p.d <= 0) { lvsa_set_error("T, P, H, d must be > 0"); return LVSA_EINVAL; }
+    if (p.B == 0) p.B = 1;
+    if (p.B < 0) { lvsa_set_error("B must be > 0"); return LVSA_EINVAL; }
+    if (p.window < 0) { lvsa_set_error("window must be >= 0"); return LVSA_EINVAL; }
+    if (p.anchors < LVSA_ANCHORS_ALL_TILES) { lvsa_set_error("anchors must be >= -1"); return LVSA_EINVAL; }
+    if (p.step < 0 || p.layer < 0) { lvsa_set_error("step and layer must be >= 0"); return LVSA_EINVAL; }
+    if ((long long)p.T * p.P >= (1ll << 31)) { lvsa_set_error("T*P must be < 2^31"); return LVSA_EINVAL; }
+    if (p.tie_break != LVSA_TIE_LO && p.tie_break != LVSA_TIE_HI) { lvsa_set_error("bad tie_break"); return LVSA_EINVAL; }
+    if (p.dtype != LVSA_DTYPE_BF16 && p.dtype != LVSA_DTYPE_FP32) { lvsa_set_error("bad dtype"); return LVSA_EINVAL; }
+    if (p.kernel < LVSA_KERNEL_AUTO || p.kernel > LVSA_KERNEL_TCGEN05) { lvsa_set_error("bad kernel"); return LVSA_EINVAL; }
+    if (p.T > 4096) { lvsa_set_error("T > 4096 frames is not supported"); return LVSA_EUNSUPPORTED; }
+    if (p.d != 64 && p.d != 128) { lvsa_set_error("head dim must be 64 or 128"); return LVSA_EUNSUPPORTED; }
+    if (p.tile_q == 0) p.tile_q = p.d;
+    if (p.tile_k == 0) p.tile_k = p.d;
+    if (p.tile_q != p.d || p.tile_k != p.d) {
+        lvsa_set_error("tiles must be 128x128 for d = 128 and 64x64 for d = 64");
+        return LVSA_EUNSUPPORTED;
+    }
+    if (p.dtype == LVSA_DTYPE_FP32 && p.kernel == LVSA_KERNEL_TCGEN05) {
+        lvsa_set_error("the tcgen05 kernel takes bf16 only");
+        return LVSA_EUNSUPPORTED;
+    }
+    if (!(p.softmax_scale > 0.f)) p.softmax_scale = 1.0f / sqrtf((float)p.d);
+
+    lvsa_index *ix = new (std::nothrow) lvsa_index();
+    if (ix == nullptr) { lvsa_set_error("out of host memory"); return LVSA_ENOMEM; }
+    ix->p = p;
+    ix->N = (int64_t)p.T * p.P;
+    ix->nq = (int32_t)((ix->N + p.tile_q - 1) / p.tile_q);
+    ix->nk = (int32_t)((ix->N + p.tile_k - 1) / p.tile_k);
+    ix->words = (p.T + 31) / 32;
+    ix->group = 2;
+    if ((long long)ix->nq * ix->nk >= (1ll << 31)) {
+        lvsa_index_destroy(ix);
+        lvsa_set_error("nq*nk must be < 2^31");
+        return LVSA_EUNSUPPORTED;
+    }
+    cudaError_t e = cudaGetDevice(&ix->device);
+    if (e != cudaSuccess) { lvsa_index_destroy(ix); return lvsa_cuda_fail(e, "cudaGetDevice (no usable CUDA device; there is no CPU fallback)"); }
+    lvsa_status_t st = lvsa_index_build_device(ix, (cudaStream_t)stream);
+    if (st != LVSA_OK) { lvsa_index_destroy(ix); return st; }
+    if (use_tcgen05(ix) && !lvsa_attn_sm100_supported(ix)) {
+        lvsa_index_destroy(ix);
+        lvsa_set_error("tcgen05 kernel: device is not sm_100 or shape unsupported");
+        return LVSA_EUNSUPPORTED;
+    }
+    *out = ix;
+    return LVSA_OK;
+}
+
+lvsa_index_t *lvsa_build_block_index(int T, int P, int H, int d, int window, int anchors, int step,
+                                     int layer) {
+    lvsa_params_t p;
+    memset(&p, 0, sizeof(p));
+    p.T = T; p.P = P; p.H = H; p.d = d; p.window = window; p.anchors = anchors; p.step = step;
+    p.layer = layer;
+    lvsa_index_t *ix = nullptr;
+    if (lvsa_build_block_index_ex(&p, nullptr, &ix) != LVSA_OK) return nullptr;
+    return ix;
+}
+
+lvsa_status_t lvsa_attn_fwd(const void *q, const void *k, const void *v, const lvsa_index_t *index,
+                            void *out, float *lse, void *stream) {
+    if (q == nullptr || k == nullptr || v == nullptr || index == nullptr || out == nullptr) {
+        lvsa_set_error("NULL argument");
+        return LVSA_EINVAL;
+    }
+    if (((uintptr_t)q | (uintptr_t)k | (uintptr_t)v | (uintptr_t)out) & 15u) {
+        lvsa_set_error("q, k, v, out must be 16-byte aligned");
+        return LVSA_EINVAL;
+    }
+    if (use_tcgen05(index)) return lvsa_attn_sm100_launch(index, q, k, v, out, lse, (cudaStream_t)stream);
+    return lvsa_attn_simt_launch(index, q, k, v, out, lse, (cudaStream_t)stream);
+}
+
+lvsa_status_t lvsa_attn_fwd_host(const void *qh, const void *kh, const void *vh, lvsa_index_t *ix,
+                                 void *oh, float *lseh, void *stream_) {
+    if (qh == nullptr || kh == nullptr || vh == nullptr || ix == nullptr || oh == nullptr) {
+        lvsa_set_error("NULL argument");
+        return LVSA_EINVAL;
+    }
+    cudaStream_t stream = (cudaStream_t)stream_;
+    const size_t bytes = (size_t)ix->p.B * ix->N * ix->p.H * ix->p.d * elem_size(ix);
+    const size_t lbytes = sizeof(float) * (size_t)ix->p.B * ix->p.H * ix->N;
+    if (ix->s_q == nullptr) {
+        LVSA_CUDA_TRY(cudaMalloc(&ix->s_q, bytes));
+        LVSA_CUDA_TRY(cudaMalloc(&ix->s_k, bytes));
+        LVSA_CUDA_TRY(cudaMalloc(&ix->s_v, bytes));
+        LVSA_CUDA_TRY(cudaMalloc(&ix->s_o, bytes));
+        LVSA_CUDA_TRY(cudaMalloc(&ix->s_lse, lbytes));
+    }
+    LVSA_CUDA_TRY(cudaMemcpyAsync(ix->s_q, qh, bytes, cudaMemcpyHostToDevice, stream));
+    LVSA_CUDA_TRY(cudaMemcpyAsync(ix->s_k, kh, bytes, cudaMemcpyHostToDevice, stream));
+    LVSA_CUDA_TRY(cudaMemcpyAsync(ix->s_v, vh, bytes, cudaMemcpyHostToDevice, stream));
+    lvsa_status_t st = lvsa_attn_fwd(ix->s_q, ix->s_k, ix->s_v, ix, ix->s_o, ix->s_lse, stream);
+    if (st != LVSA_OK) return st;
+    LVSA_CUDA_TRY(cudaMemcpyAsync(oh, ix->s_o, bytes, cudaMemcpyDeviceToHost, stream));
+    if (lseh != nullptr) LVSA_CUDA_TRY(cudaMemcpyAsync(lseh, ix->s_lse, lbytes, cudaMemcpyDeviceToHost, stream));
+    LVSA_CUDA_TRY(cudaStreamSynchronize(stream));
+    return LVSA_OK;
+}
+
+void lvsa_index_destroy(lvsa_index_t *ix) {
+    if (ix == nullptr) return;
+    cudaFree(ix->d_wlo); cudaFree(ix->d_whi); cudaFree(ix->d_abits); cudaFree(ix->d_meta);
+    cudaFree(ix->d_indptr); cudaFree(ix->d_indices); cudaFree(ix->d_flags);
+    cudaFree(ix->d_item_ptr); cudaFree(ix->d_item_tiles);
+    cudaFree(ix->s_q); cudaFree(ix->s_k); cudaFree(ix->s_v); cudaFree(ix->s_o); cudaFree(ix->s_lse);
+    delete ix;
+}
+
+lvsa_status_t lvsa_index_info(const lvsa_index_t *ix, lvsa_index_info_t *info) {
+    if (ix == nullptr || info == nullptr) { lvsa_set_error("NULL argument"); return LVSA_EINVAL; }
+    memset(info, 0, sizeof(*info));
+    const lvsa_params_t &p = ix->p;
+    info->T = p.T; info->P = p.P; info->H = p.H; info->d = p.d; info->B = p.B;
+    info->window = p.window; info->anchors = p.anchors; info->step = p.step; info->layer = p.layer;
+    info->tile_q = p.tile_q; info->tile_k = p.tile_k; info->nq = ix->nq; info->nk = ix->nk;
+    info->T_per = ix->T_per; info->phase = ix->phase; info->n_global = ix->n_global;
+    info->words = ix->words; info->dtype = p.dtype;
+    info->kernel = use_tcgen05(ix) ? LVSA_KERNEL_TCGEN05 : LVSA_KERNEL_SIMT;
+    info->N = ix->N; info->nnz = ix->nnz; info->n_partial = ix->n_partial;
+    info->n_items = ix->n_items; info->n_item_tiles = ix->n_item_tiles;
+    return LVSA_OK;
+}
+
+lvsa_status_t lvsa_index_copy_host(const lvsa_index_t *ix, int32_t *indptr, int32_t *indices,
+                                   uint8_t *flags, int32_t *w_lo, int32_t *w_hi, uint32_t *a_bits) {
+    if (ix == nullptr) { lvsa_set_error("NULL index"); return LVSA_EINVAL; }
+    const int T = ix->p.T;
+    if (indptr) LVSA_CUDA_TRY(cudaMemcpy(indptr, ix->d_indptr, sizeof(int32_t) * ((size_t)ix->nq + 1), cudaMemcpyDeviceToHost));
+    if (indices && ix->nnz) LVSA_CUDA_TRY(cudaMemcpy(indices, ix->d_indices, sizeof(int32_t) * (size_t)ix->nnz, cudaMemcpyDeviceToHost));
+    if (flags && ix->nnz) LVSA_CUDA_TRY(cudaMemcpy(flags, ix->d_flags, (size_t)ix->nnz, cudaMemcpyDeviceToHost));
+    if (w_lo) LVSA_CUDA_TRY(cudaMemcpy(w_lo, ix->d_wlo, sizeof(int32_t) * T, cudaMemcpyDeviceToHost));
+    if (w_hi) LVSA_CUDA_TRY(cudaMemcpy(w_hi, ix->d_whi, sizeof(int32_t) * T, cudaMemcpyDeviceToHost));
+    if (a_bits) LVSA_CUDA_TRY(cudaMemcpy(a_bits, ix->d_abits, sizeof(uint32_t) * (size_t)T * ix->words, cudaMemcpyDeviceToHost));
+    return LVSA_OK;
+}
+
+int lvsa_attn_fwd_launches(const lvsa_index_t *ix) { return ix == nullptr ? 0 : 1; }
+
+}  // extern "C"

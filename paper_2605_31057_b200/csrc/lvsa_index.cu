@@ -1,0 +1,252 @@
+// GPU index builder: steps a1-a5 of the hot path.
+//   lvsa_frames_kernel : T_per, G^s (Eq. 3), adaptive window,
+//                        Algorithm 1, A(t) bitsets (Def. 2)
+//   lvsa_tiles_kernel  : frame -> token -> tile mapping, count then fill (CSR + FULL/PARTIAL)
+//   lvsa_scan_kernel   : exclusive scan of the per-tile counts
+//   lvsa_items_kernel  : merges the lists of adjacent q tiles into the attention kernel's
+//                        work items (q-tile groups that share K/V loads)
+// Integer arithmetic only.  Written from the paper; shares nothing with oracle/.
+#include <limits.h>
+
+#include "lvsa_internal.h"
+
+namespace {
+
+__device__ __forceinline__ bool bit_test(const uint32_t *bits, int x) {
+    return (bits[x >> 5] >> (x & 31)) & 1u;
+}
+
+// One block.  g_bits lives in shared memory; every thread then owns frames t, t+blockDim, ...
+__global__ void lvsa_frames_kernel(int T, int W, int a, int s, int tie_hi, int words,
+                                   int32_t *__restrict__ w_lo, int32_t *__restrict__ w_hi,
+                                   uint32_t *__restrict__ a_bits, int32_t *__restrict__ meta) {
+    extern __shared__ uint32_t g_bits[];
+    __shared__ int n_global_s;
+    const int tid = threadIdx.x;
+    for (int w = tid; w < words; w += blockDim.x) g_bits[w] = 0u;
+    __syncthreads();
+    const bool all_tiles = (a == LVSA_ANCHORS_ALL_TILES);
+    int T_per = 0, phase = 0;
+    if (!all_tiles && a > 0) {
+        T_per = (T + a - 1) / a;                  // ceil(T / (C-(2W+1)))
+        const int m = (T + T_per - 1) / T_per;    // ceil(T / T_per) anchors, Eq. 3
+        phase = s % T_per;
+        for (int i = tid; i < m; i += blockDim.x) {
+            const int f = (phase + i * T_per) % T;
+            atomicOr(&g_bits[f >> 5], 1u << (f & 31));
+        }
+    }
+    __syncthreads();
+    if (tid == 0) {
+        int c = 0;
+        for (int w = 0; w < words; ++w) c += __popc(g_bits[w]);
+        n_global_s = c;
+        meta[4] = T_per; meta[5] = phase; meta[6] = c;
+    }
+    __syncthreads();
+    const int n_global = n_global_s;
+    for (int t = tid; t < T; t += blockDim.x) {
+        int l, h;
+        if (all_tiles) {
+            l = 0; h = T - 1;                     // Def. 1: A(t) = all frames
+        } else {
+            // adaptive window
+            l = max(0, min(t - W, T - 1 - 2 * W));
+            h = min(T - 1, max(t + W, 2 * W));
+            // Algorithm 1
+            const int target = min(2 * W + 1, T - n_global);
+            int nonglobal = 0;
+            for (int x = l; x <= h; ++x) nonglobal += !bit_test(g_bits, x);
+            while (nonglobal < target && (l > 0 || h < T - 1)) {
+                const int room_lo = l, room_hi = T - 1 - h;
+                int nw;
+                if (room_lo > room_hi || (room_lo == room_hi && !tie_hi)) { l -= 1; nw = l; }
+                else                                                      { h += 1; nw = h; }
+                nonglobal += !bit_test(g_bits, nw);
+            }
+        }
+        w_lo[t] = l; w_hi[t] = h;
+        for (int w = 0; w < words; ++w) {
+            // bits of [l, h] that fall into word w
+            const int b0 = max(l, 32 * w), b1 = min(h, 32 * w + 31);
+            uint32_t rm = 0u;
+            if (b0 <= b1) {
+                const int n = b1 - b0 + 1;
+                rm = (n == 32 ? 0xffffffffu : ((1u << n) - 1u)) << (b0 - 32 * w);
+            }
+            a_bits[(size_t)t * words + w] = g_bits[w] | rm;
+        }
+    }
+}
+
+// One block per q tile; threads stride over kv tiles in ascending chunks so the fill pass can
+// write in order.  FILL = false: counts[i].  FILL = true: indices/flags at indptr[i].
+template <bool FILL>
+__global__ void lvsa_tiles_kernel(long long N, int P, int Bq, int Bk, int nk, int words,
+                                  const uint32_t *__restrict__ a_bits,
+                                  const int32_t *__restrict__ indptr, int32_t *__restrict__ counts,
+                                  int32_t *__restrict__ indices, uint8_t *__restrict__ flags,
+                                  int32_t *__restrict__ meta) {
+    __shared__ int warp_tot[32];
+    __shared__ int chunk_base;
+    const int i = blockIdx.x, tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const int nwarps = blockDim.x >> 5;
+    const long long r0 = (long long)i * Bq;
+    const long long r1 = min(r0 + Bq, N) - 1;
+    const int f0 = (int)(r0 / P), f1 = (int)(r1 / P);
+    int running = 0, n_part = 0;
+    const int base = FILL ? indptr[i] : 0;
+    for (int j0 = 0; j0 < nk; j0 += blockDim.x) {
+        const int j = j0 + tid;
+        bool kept = false, part = false;
+        if (j < nk) {
+            const long long c0 = (long long)j * Bk;
+            const long long c1 = min(c0 + Bk, N) - 1;
+            const int g0 = (int)(c0 / P), g1 = (int)(c1 / P);
+            part = (c0 + Bk > N);  // columns >= N are never allowed
+            for (int tq = f0; tq <= f1; ++tq) {
+                const uint32_t *row = a_bits + (size_t)tq * words;
+                for (int tk = g0; tk <= g1; ++tk) {
+                    const bool b = bit_test(row, tk);
+                    kept |= b; part |= !b;
+                }
+            }
+        }
+        const unsigned bal = __ballot_sync(0xffffffffu, kept);
+        if (lane == 0) warp_tot[wid] = __popc(bal);
+        __syncthreads();
+        int woff = 0, tot = 0;
+        for (int w = 0; w < nwarps; ++w) { const int c = warp_tot[w]; if (w < wid) woff += c; tot += c; }
+        if (FILL && kept) {
+            const int pos = base + running + woff + __popc(bal & ((1u << lane) - 1u));
+            indices[pos] = j;
+            flags[pos] = part ? LVSA_TILE_PARTIAL : LVSA_TILE_FULL;
+            n_part += part;
+        }
+        running += tot;
+        __syncthreads();
+    }
+    if (!FILL && tid == 0) counts[i] = running;
+    if (FILL) {
+        n_part = __reduce_add_sync(0xffffffffu, n_part);
+        if (lane == 0 && n_part) atomicAdd(&meta[1], n_part);
+    }
+    (void)chunk_base;
+}
+
+// Single-block exclusive scan: out[0..n] from counts[0..n-1]; total also to *total_out.
+__global__ void lvsa_scan_kernel(const int32_t *__restrict__ counts, int n, int32_t *__restrict__ out,
+                                 int32_t *__restrict__ total_out) {
+    __shared__ int warp_tot[32];
+    __shared__ int carry_s;
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5, nwarps = blockDim.x >> 5;
+    if (tid == 0) carry_s = 0;
+    __syncthreads();
+    for (int i0 = 0; i0 < n; i0 += blockDim.x) {
+        const int i = i0 + tid;
+        const int v = (i < n) ? counts[i] : 0;
+        int incl = v;
+        for (int o = 1; o < 32; o <<= 1) {
+            const int y = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= o) incl += y;
+        }
+        if (lane == 31) warp_tot[wid] = incl;
+        __syncthreads();
+        int woff = 0, tot = 0;
+        for (int w = 0; w < nwarps; ++w) { const int c = warp_tot[w]; if (w < wid) woff += c; tot += c; }
+        const int carry = carry_s;
+        if (i < n) out[i] = carry + woff + incl - v;
+        __syncthreads();
+        if (tid == 0) carry_s = carry + tot;
+        __syncthreads();
+    }
+    if (tid == 0) { out[n] = carry_s; *total_out = carry_s; }
+}
+
+// One thread per work item: union of the kv-tile lists of `group` (1 or 2) adjacent q tiles,
+// ascending, each entry tagged with the per-q-tile state (skip / full / partial).
+template <bool FILL>
+__global__ void lvsa_items_kernel(int nq, int group, long long n_items,
+                                  const int32_t *__restrict__ indptr,
+                                  const int32_t *__restrict__ indices,
+                                  const uint8_t *__restrict__ flags,
+                                  const int32_t *__restrict__ item_ptr, int32_t *__restrict__ counts,
+                                  int32_t *__restrict__ item_tiles) {
+    const long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (g >= n_items) return;
+    const int i0 = (int)(g * group), i1 = i0 + 1;
+    int a = indptr[i0], ae = indptr[i0 + 1];
+    int b = 0, be = 0;
+    if (group == 2 && i1 < nq) { b = indptr[i1]; be = indptr[i1 + 1]; }
+    int pos = FILL ? item_ptr[g] : 0, cnt = 0;
+    while (a < ae || b < be) {
+        const int ja = (a < ae) ? indices[a] : INT_MAX;
+        const int jb = (b < be) ? indices[b] : INT_MAX;
+        const int j = min(ja, jb);
+        int st0 = LVSA_ST_SKIP, st1 = LVSA_ST_SKIP;
+        if (ja == j) { st0 = flags[a] ? LVSA_ST_PARTIAL : LVSA_ST_FULL; ++a; }
+        if (jb == j) { st1 = flags[b] ? LVSA_ST_PARTIAL : LVSA_ST_FULL; ++b; }
+        if (FILL) item_tiles[pos + cnt] = j | (st0 << LVSA_ITEM_J_BITS) | (st1 << (LVSA_ITEM_J_BITS + 2));
+        ++cnt;
+    }
+    if (!FILL) counts[g] = cnt;
+}
+
+}  // namespace
+
+lvsa_status_t lvsa_index_build_device(lvsa_index *ix, cudaStream_t stream) {
+    const lvsa_params_t &p = ix->p;
+    const int T = p.T, words = ix->words;
+    LVSA_CUDA_TRY(cudaMalloc(&ix->d_wlo, sizeof(int32_t) * T));
+    LVSA_CUDA_TRY(cudaMalloc(&ix->d_whi, sizeof(int32_t) * T));
+    LVSA_CUDA_TRY(cudaMalloc(&ix->d_abits, sizeof(uint32_t) * (size_t)T * words));
+    LVSA_CUDA_TRY(cudaMalloc(&ix->d_meta, sizeof(int32_t) * 8));
+    LVSA_CUDA_TRY(cudaMemsetAsync(ix->d_meta, 0, sizeof(int32_t) * 8, stream));
+    LVSA_CUDA_TRY(cudaMalloc(&ix->d_indptr, sizeof(int32_t) * ((size_t)ix->nq + 1)));
+    int32_t *d_counts = nullptr;
+    LVSA_CUDA_TRY(cudaMalloc(&d_counts, sizeof(int32_t) * ((size_t)ix->nq + 1)));
+
+    const int W = p.window > T ? T : p.window;  // W >= T already spans [0, T-1]; avoids 2W overflow
+    lvsa_frames_kernel<<<1, 256, sizeof(uint32_t) * words, stream>>>(
+        T, W, p.anchors, p.step, p.tie_break == LVSA_TIE_HI, words, ix->d_wlo, ix->d_whi,
+        ix->d_abits, ix->d_meta);
+    lvsa_tiles_kernel<false><<<ix->nq, 256, 0, stream>>>(
+        (long long)ix->N, p.P, p.tile_q, p.tile_k, ix->nk, words, ix->d_abits, nullptr, d_counts,
+        nullptr, nullptr, ix->d_meta);
+    lvsa_scan_kernel<<<1, 1024, 0, stream>>>(d_counts, ix->nq, ix->d_indptr, ix->d_meta + 0);
+    int32_t meta[8];
+    LVSA_CUDA_TRY(cudaMemcpyAsync(meta, ix->d_meta, sizeof(meta), cudaMemcpyDeviceToHost, stream));
+    LVSA_CUDA_TRY(cudaStreamSynchronize(stream));  // the one sync: learn nnz
+    LVSA_CUDA_TRY(cudaGetLastError());
+    ix->nnz = meta[0];
+    ix->T_per = meta[4]; ix->phase = meta[5]; ix->n_global = meta[6];
+    const size_t nnz_alloc = ix->nnz > 0 ? (size_t)ix->nnz : 1;
+    LVSA_CUDA_TRY(cudaMalloc(&ix->d_indices, sizeof(int32_t) * nnz_alloc));
+    LVSA_CUDA_TRY(cudaMalloc(&ix->d_flags, nnz_alloc));
+    lvsa_tiles_kernel<true><<<ix->nq, 256, 0, stream>>>(
+        (long long)ix->N, p.P, p.tile_q, p.tile_k, ix->nk, words, ix->d_abits, ix->d_indptr, nullptr,
+        ix->d_indices, ix->d_flags, ix->d_meta);
+
+    // work items for the attention kernel
+    ix->n_items = (ix->nq + ix->group - 1) / ix->group;
+    LVSA_CUDA_TRY(cudaMalloc(&ix->d_item_ptr, sizeof(int32_t) * ((size_t)ix->n_items + 1)));
+    const int ib = 128, ig = (int)((ix->n_items + ib - 1) / ib);
+    lvsa_items_kernel<false><<<ig, ib, 0, stream>>>(ix->nq, ix->group, (long long)ix->n_items,
+                                                     ix->d_indptr, ix->d_indices, ix->d_flags,
+                                                     nullptr, d_counts, nullptr);
+    lvsa_scan_kernel<<<1, 1024, 0, stream>>>(d_counts, (int)ix->n_items, ix->d_item_ptr,
+                                             ix->d_meta + 2);
+    LVSA_CUDA_TRY(cudaMemcpyAsync(meta, ix->d_meta, sizeof(meta), cudaMemcpyDeviceToHost, stream));
+    LVSA_CUDA_TRY(cudaStreamSynchronize(stream));
+    ix->n_partial = meta[1];
+    ix->n_item_tiles = meta[2];
+    LVSA_CUDA_TRY(cudaMalloc(&ix->d_item_tiles,
+                             sizeof(int32_t) * (ix->n_item_tiles > 0 ? (size_t)ix->n_item_tiles : 1)));
+    lvsa_items_kernel<true><<<ig, ib, 0, stream>>>(ix->nq, ix->group, (long long)ix->n_items,
+                                                    ix->d_indptr, ix->d_indices, ix->d_flags,
+                                                    ix->d_item_ptr, nullptr, ix->d_item_tiles);
+    LVSA_CUDA_TRY(cudaStreamSynchronize(stream));
+    LVSA_CUDA_TRY(cudaGetLastError());
+    cudaFree(d_counts);
+    return LVSA_OK;
+}

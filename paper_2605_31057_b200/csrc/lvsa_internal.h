@@ -1,0 +1,62 @@
+// Internal declarations of liblvsa (CUDA path).  Not part of the C ABI; include/lvsa.h is.
+// Nothing here is shared with oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+
+#include "lvsa.h"
+
+// Work-item entry encoding for the attention kernels (one int32 per kv-tile visit of a q-tile
+// group).  bits [0,26): kv tile j.  bits [26,28): state for the group's q tile 0, bits [28,30):
+// state for q tile 1.  States:
+constexpr int LVSA_ST_SKIP = 0, LVSA_ST_FULL = 1, LVSA_ST_PARTIAL = 2;
+constexpr int LVSA_ITEM_J_BITS = 26;
+constexpr int LVSA_ITEM_J_MASK = (1 << LVSA_ITEM_J_BITS) - 1;
+
+struct lvsa_index {
+    lvsa_params_t p;  // with defaults resolved
+    int64_t N = 0;
+    int32_t nq = 0, nk = 0, words = 0;
+    int32_t T_per = 0, phase = 0, n_global = 0;
+    int64_t nnz = 0, n_partial = 0;
+    int device = 0;
+    // device buffers (owned)
+    int32_t *d_wlo = nullptr, *d_whi = nullptr;
+    uint32_t *d_abits = nullptr;   // [T][words]
+    int32_t *d_meta = nullptr;     // small scratch: {nnz, n_partial, n_item_tiles, n_global}
+    int32_t *d_indptr = nullptr;   // [nq+1]
+    int32_t *d_indices = nullptr;  // [nnz]
+    uint8_t *d_flags = nullptr;    // [nnz]
+    // attention work items: groups of LVSA_GROUP adjacent q tiles that share kv-tile loads
+    int32_t group = 2;
+    int64_t n_items = 0, n_item_tiles = 0;
+    int32_t *d_item_ptr = nullptr;    // [n_items+1]
+    int32_t *d_item_tiles = nullptr;  // [n_item_tiles], encoding above
+    // scratch for lvsa_attn_fwd_host (allocated on first use)
+    void *s_q = nullptr, *s_k = nullptr, *s_v = nullptr, *s_o = nullptr;
+    float *s_lse = nullptr;
+};
+
+void lvsa_set_error(const std::string &msg);
+lvsa_status_t lvsa_cuda_fail(cudaError_t e, const char *what);
+
+#define LVSA_CUDA_TRY(expr)                                          \
+    do {                                                             \
+        cudaError_t _e = (expr);                                     \
+        if (_e != cudaSuccess) return lvsa_cuda_fail(_e, #expr);     \
+    } while (0)
+
+// lvsa_index.cu
+lvsa_status_t lvsa_index_build_device(lvsa_index *ix, cudaStream_t stream);
+
+// lvsa_attn_simt.cu
+lvsa_status_t lvsa_attn_simt_launch(const lvsa_index *ix, const void *q, const void *k,
+                                    const void *v, void *out, float *lse, cudaStream_t stream);
+
+// lvsa_attn_sm100.cu
+lvsa_status_t lvsa_attn_sm100_launch(const lvsa_index *ix, const void *q, const void *k,
+                                     const void *v, void *out, float *lse, cudaStream_t stream);
+int lvsa_attn_sm100_supported(const lvsa_index *ix);

@@ -1,0 +1,127 @@
+"""Attention parity, CUDA path (through the C ABI) vs the fp64 oracle, element by element."""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+from helpers import (BF16_MAX_ABS, BF16_MEAN_ABS, FP32_MAX_ABS, LSE_MAX_ABS_BF16, LSE_MAX_ABS_FP32,
+                     build_index, compare, gpu_attn, oracle_attn)
+from oracle import lvsa_oracle as orc
+from paper_2605_31057_b200 import binding, inputs
+
+pytestmark = pytest.mark.gpu
+
+KERNELS = {"tcgen05": dict(dtype=binding.DTYPE_BF16, kernel=binding.KERNEL_TCGEN05),
+           "simt_bf16": dict(dtype=binding.DTYPE_BF16, kernel=binding.KERNEL_SIMT),
+           "simt_fp32": dict(dtype=binding.DTYPE_FP32, kernel=binding.KERNEL_SIMT)}
+
+
+def tol(kname):
+    if kname == "simt_fp32":
+        return FP32_MAX_ABS, FP32_MAX_ABS, LSE_MAX_ABS_FP32
+    if kname == "simt_bf16":
+        # fp32 math, but the output is rounded to bf16: half an ulp at |out| < 1 is 2^-9
+        return BF16_MAX_ABS, BF16_MEAN_ABS, LSE_MAX_ABS_FP32
+    return BF16_MAX_ABS, BF16_MEAN_ABS, LSE_MAX_ABS_BF16
+
+
+def run_case(w, kname, steps, rows=None, layer=0, anchors=None, window=None, seed=None):
+    torch_dtype = torch.float32 if kname == "simt_fp32" else torch.bfloat16
+    q, k, v = inputs.make_qkv(w, "cuda", torch_dtype, seed=seed)
+    rows = np.arange(w.N) if rows is None else rows
+    mx, mean, lse_tol = tol(kname)
+    for s in steps:
+        ix = build_index(w, s, layer, anchors=anchors, window=window, **KERNELS[kname])
+        out, lse = gpu_attn(w, ix, q, k, v)
+        for b in range(w.B):
+            ref, ref_lse = oracle_attn(w, q, k, v, s, rows, anchors=anchors, window=window, b=b)
+            st = compare(out, lse, ref, ref_lse, rows, b)
+            assert st["nan"] == 0, (kname, s, st)
+            assert st["max_abs"] <= mx and st["mean_abs"] <= mean, (kname, s, st)
+            assert st["lse_max_abs"] <= lse_tol, (kname, s, st)
+        ix.destroy()
+
+
+# ---------------------------------------------------------------- config 1 (tiny), all rows
+@pytest.mark.parametrize("kname", ["simt_fp32", "simt_bf16", "tcgen05"])
+def test_tiny_all_steps_layers(kname):
+    w = inputs.WORKLOADS["tiny"]
+    for layer in w.layers:
+        run_case(w, kname, w.steps if layer == 0 else w.steps[:4], layer=layer)
+
+
+@pytest.mark.parametrize("kname", ["simt_fp32", "simt_bf16", "tcgen05"])
+@pytest.mark.parametrize("name", ["tiny_straddle", "small128"])
+def test_straddling_tiles_all_rows(name, kname):
+    w = inputs.WORKLOADS[name]
+    run_case(w, kname, w.steps[:5])
+
+
+@pytest.mark.parametrize("kname", ["simt_fp32", "tcgen05"])
+def test_edge_shapes(kname):
+    W = inputs.Workload
+    cases = [W("one_frame", 1, T=1, P=100, H=1, d=64, tile=64, W=0, a=0),           # single ragged tile
+             W("one_tile", 1, T=1, P=128, H=2, d=128, tile=128, W=0, a=0),
+             W("odd_nq", 1, T=3, P=128, H=1, d=128, tile=128, W=0, a=1),            # nq = 3: lone last q tile
+             W("tiny_frames", 1, T=40, P=7, H=1, d=64, tile=64, W=1, a=3),          # many frames per tile
+             W("batch2", 1, T=6, P=70, H=2, d=64, tile=64, W=1, a=2, B=2),
+             W("dense_window", 1, T=5, P=90, H=2, d=128, tile=128, W=2, a=0),       # 2W+1 >= T: Eq. 1
+             W("all_anchors", 1, T=6, P=60, H=1, d=64, tile=64, W=0, a=6)]
+    for w in cases:
+        run_case(w, kname, (0, 1, 2))
+    run_case(cases[3], kname, (0,), anchors=binding.ALL_TILES)
+
+
+# ---------------------------------------------------------------- closed-form probe (P14), any size
+def probe_check(w, kname, steps):
+    q, k, v = inputs.probe_qkv(w, "cuda", torch.bfloat16)
+    for s in steps:
+        ix = build_index(w, s, **KERNELS[kname])
+        out, lse = gpu_attn(w, ix, q, k, v)
+        host = ix.copy_host()
+        A = ((host.a_bits[:, :, None] >> np.arange(32, dtype=np.uint32)[None, None, :]) & 1)
+        A = A.reshape(w.T, -1)[:, :w.T].astype(np.float64)          # A(t) as the GPU index holds it
+        p = orc.pattern(w.T, w.W, w.a, s)
+        assert np.array_equal(A, p.A.astype(np.float64))
+        cnt = p.A.sum(1).astype(np.float64)
+        want = np.zeros((w.T, w.d))
+        want[:, :w.T] = p.A / cnt[:, None]                           # [c in A(t)] / |A(t)|
+        want_t = torch.from_numpy(want).to("cuda")
+        frame = torch.arange(w.N, device="cuda") // w.P
+        err = (out[0].double() - want_t[frame][:, None, :]).abs()
+        # 1/|A| in bf16: relative 2^-9; P entries are exactly 1 so only output rounding remains
+        assert float(err.max()) <= 2e-3 * float(want.max()) + 1e-6, (s, float(err.max()))
+        want_lse = torch.log(torch.from_numpy(cnt * w.P)).to("cuda")[frame]
+        assert float((lse[0].double() - want_lse[None, :]).abs().max()) <= 1e-4
+        ix.destroy()
+
+
+@pytest.mark.parametrize("name", ["tiny", "tiny_straddle", "small128", "wan1.3b_1x"])
+def test_closed_form_probe(name):
+    w = inputs.WORKLOADS[name]
+    probe_check(w, "tcgen05", w.steps[:4])
+
+
+# ---------------------------------------------------------------- configs 2-5, sampled rows
+@pytest.mark.slow
+@pytest.mark.parametrize("name,n_rows", [("wan1.3b_1x", 4096), ("wan1.3b_6x", 4096),
+                                         ("hv1.5_2x", 4096), ("wan14b_6x", 4096)])
+def test_large_configs_sampled_rows(name, n_rows):
+    w = inputs.WORKLOADS[name]
+    rows = inputs.sample_rows(w, n_uniform=n_rows - 512, n_edge=512)
+    # one oracle pass per distinct phase (steps 25 and 49 share s mod T_per on these configs)
+    steps, seen = [], set()
+    for s in w.steps:
+        ph = orc.pattern(w.T, w.W, w.a, s).phase
+        if ph not in seen:
+            seen.add(ph); steps.append(s)
+    run_case(w, "tcgen05", steps, rows=rows, layer=w.layers[0])
+
+
+@pytest.mark.slow
+def test_wan6x_probe_and_all_tiles():
+    w = inputs.WORKLOADS["wan1.3b_6x"]
+    probe_check(w, "tcgen05", (0, 25))
+    rows = inputs.sample_rows(w, n_uniform=448, n_edge=64)
+    run_case(w, "tcgen05", (0,), rows=rows, anchors=binding.ALL_TILES)
