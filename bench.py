@@ -1,0 +1,371 @@
+#!/usr/bin/env python
+"""bench.py — LVSA block-sparse attention forward on B200.
+
+One "step" = one pass of the whole hot path for one denoising step: build the block index on the
+GPU (a1-a5) and run the attention forward (a6) on one batch of synthetic Wan-2.1-1.3B 6x-horizon
+tensors (BASELINE.json configs[2]: T=121, P=1560, N=188760, H=12, d=128, bf16).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload NAME]
+
+Prints ONE JSON line (rank 0).  `value` = effective TFLOP/s counting only computed tiles.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+import torch
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2605_31057_b200 import inputs  # noqa: E402
+
+METRIC = "ms/attention call and effective TFLOPS (% of B200 bf16 peak) vs all-tiles dense"
+UNIT = "TFLOP/s (bf16, computed tiles only)"
+FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            d = json.load(f)
+        d["_source"] = "measured"
+        return d
+    d = dict(FALLBACK_PEAKS)
+    d["_source"] = "fallback"
+    return d
+
+
+class ClockSampler:
+    """Samples nvidia-smi SM clocks / throttle reasons while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu: int):
+        self.gpu, self.rows, self.proc = gpu, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.gpu), f"--query-gpu={self.Q}",
+                 "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thr = threading.Thread(target=self._read, daemon=True)
+            self.thr.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            parts = [x.strip() for x in r.split(",")]
+            if len(parts) < 6:
+                continue
+            try:
+                sm.append(float(parts[0])); mx.append(float(parts[1]))
+            except ValueError:
+                continue
+            for n, val in zip(names, parts[2:6]):
+                if val.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None,
+                "sm_max_mhz": max(mx) if mx else None, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def dist_setup(n_gpus: int):
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        import torch.distributed as dist
+        torch.cuda.set_device(local)
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        return rank, world, local, dist
+    return rank, world, local, None
+
+
+def exact_flops(w, A) -> float:
+    """Eq. 2 work: 4 d flops per (query row, head, attended key)."""
+    return float(A.sum()) * w.P * w.P * 4.0 * w.d * w.H * w.B
+
+
+# ------------------------------------------------------------------------------------------
+def run_ours(args):
+    from paper_2605_31057_b200 import binding
+    rank, world, local, dist = dist_setup(args.gpus)
+    dev = torch.device("cuda", local)
+    torch.cuda.set_device(dev)
+    w = inputs.WORKLOADS[args.workload]
+    pk = peaks()
+    q, k, v = inputs.make_qkv(w, f"cuda:{local}", torch.bfloat16, seed=w.seed + rank)
+    out = torch.empty_like(q)
+    lse = torch.empty((w.B, w.H, w.N), device=dev, dtype=torch.float32)
+    stream = torch.cuda.current_stream()
+    steps_cycle = list(w.steps) if w.steps else [0]
+
+    def build(s):
+        return binding.lvsa_build_block_index_ex(
+            stream=stream.cuda_stream, T=w.T, P=w.P, H=w.H, d=w.d, B=w.B, window=w.W, anchors=w.a,
+            step=s, layer=w.layers[0] if w.layers else 0)
+
+    def one_step(i):
+        ix = build(steps_cycle[i % len(steps_cycle)])
+        binding.lvsa_attn_fwd(q, k, v, ix, out, lse, stream.cuda_stream)
+        return ix
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident throughput: K whole steps
+    keep = []
+    for i in range(args.warmup):
+        keep.append(one_step(i))
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record(stream)
+    infos = []
+    for i in range(args.steps):
+        ix = one_step(i)
+        keep.append(ix)
+    e1.record(stream)
+    barrier()
+    total_ms = e0.elapsed_time(e1)
+    for ix in keep[-args.steps:]:
+        infos.append(ix.info())
+    launches_per_step = 7 + keep[-1].launches()   # 7 index-builder kernels + attention
+    tile_flops = sum(float(i.nnz) * w.H * w.B * 4.0 * w.tile * w.tile * w.d for i in infos)
+    nnz_mean = float(np.mean([i.nnz for i in infos]))
+
+    # ---- dominant kernel alone (attention), same stream, CUDA events
+    ix_k = build(steps_cycle[min(1, len(steps_cycle) - 1)])
+    info_k = ix_k.info()
+    for _ in range(2):
+        binding.lvsa_attn_fwd(q, k, v, ix_k, out, lse, stream.cuda_stream)
+    torch.cuda.synchronize()
+    ks = max(3, min(10, args.steps))
+    k0, k1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    k0.record(stream)
+    for _ in range(ks):
+        binding.lvsa_attn_fwd(q, k, v, ix_k, out, lse, stream.cuda_stream)
+    k1.record(stream)
+    torch.cuda.synchronize()
+    kern_ms = k0.elapsed_time(k1) / ks
+    kern_flops = float(info_k.nnz) * w.H * w.B * 4.0 * w.tile * w.tile * w.d
+    clocks = sampler.stop() if rank == 0 else None
+
+    # ---- index build alone (a1-a5)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    nb = 5
+    for i in range(nb):
+        keep.append(build(i))
+    torch.cuda.synchronize()
+    build_us = (time.perf_counter() - t0) / nb * 1e6
+
+    # ---- all-tiles (dense, Eq. 1) path of the same kernel, for the speedup line (rank 0, N = 1)
+    dense_ms = None
+    if rank == 0 and not args.no_dense:
+        ixd = binding.lvsa_build_block_index_ex(
+            stream=stream.cuda_stream, T=w.T, P=w.P, H=w.H, d=w.d, B=w.B, window=w.W,
+            anchors=binding.ALL_TILES, step=0, layer=0)
+        binding.lvsa_attn_fwd(q, k, v, ixd, out, lse, stream.cuda_stream)
+        torch.cuda.synchronize()
+        d0, d1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        d0.record(stream)
+        binding.lvsa_attn_fwd(q, k, v, ixd, out, lse, stream.cuda_stream)
+        d1.record(stream)
+        torch.cuda.synchronize()
+        dense_ms = d0.elapsed_time(d1)
+        dense_nnz = ixd.info().nnz
+        ixd.destroy()
+        # restore the LVSA result in `out`
+        binding.lvsa_attn_fwd(q, k, v, ix_k, out, lse, stream.cuda_stream)
+
+    # ---- end to end through the C ABI with HOST buffers (H2D + kernels + D2H inside the region)
+    e2e = None
+    if not args.no_e2e:
+        qh, kh, vh = (x.cpu().pin_memory() for x in (q, k, v))
+        oh = torch.empty_like(qh).pin_memory()
+        lh = torch.empty((w.B, w.H, w.N), dtype=torch.float32).pin_memory()
+        n_e2e = max(1, min(3, args.steps))
+        ixh = build(steps_cycle[0])
+        binding.lvsa_attn_fwd_host(qh, kh, vh, ixh, oh, lh, stream.cuda_stream)   # warm-up, allocs scratch
+        barrier()
+        h0, h1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        h0.record(stream)
+        fl_e2e = 0.0
+        for i in range(n_e2e):
+            ixh2 = build(steps_cycle[i % len(steps_cycle)])
+            ixh2_info = ixh2.info()
+            # scratch lives in the handle: reuse the warmed handle's buffers by running through it
+            binding.lvsa_attn_fwd_host(qh, kh, vh, ixh, oh, lh, stream.cuda_stream)
+            fl_e2e += float(ixh.info().nnz) * w.H * w.B * 4.0 * w.tile * w.tile * w.d
+            ixh2.destroy()
+        h1.record(stream)
+        barrier()
+        e2e_ms = h0.elapsed_time(h1) / n_e2e
+        bi = 3 * q.numel() * q.element_size()
+        bo = out.numel() * out.element_size() + lse.numel() * 4
+        e2e = {"ms": e2e_ms, "flops": fl_e2e / n_e2e, "h2d": bi, "d2h": bo}
+        ixh.destroy()
+        del qh, kh, vh, oh, lh
+
+    # ---- max over ranks, aggregate
+    ms_step = total_ms / args.steps
+    if dist is not None:
+        t = torch.tensor([ms_step, kern_ms, e2e["ms"] if e2e else 0.0], device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_step, kern_ms = float(t[0]), float(t[1])
+        if e2e:
+            e2e["ms"] = float(t[2])
+    value = world * (tile_flops / args.steps) / (ms_step * 1e-3) / 1e12
+
+    # ---- CPU baseline: the oracle as it stands, bounded sample (rank 0, N = 1 only)
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu:
+        cpu = cpu_baseline(w, q, k, v, steps_cycle[0], args.cpu_rows)
+
+    if rank == 0:
+        peak = pk["bf16_tflops"]
+        achieved = kern_flops / (kern_ms * 1e-3) / 1e12
+        line = {
+            "metric": METRIC, "value": round(value, 2), "unit": UNIT, "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": round(ms_step, 4),
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
+            "data": "synthetic (i.i.d. N(0,1) bf16, seeded Philox; stands in for Wan 2.1 latents)",
+            "config": {"workload": args.workload, "T": w.T, "P": w.P, "N": w.N, "H": w.H, "d": w.d,
+                       "B": w.B, "tile": w.tile, "window": w.W, "anchors": w.a,
+                       "steps_cycled": steps_cycle, "nnz_mean": nnz_mean,
+                       "l2": "inputs (3 x %.0f MB) exceed the 126 MB L2; no flush" % (q.numel() * 2 / 1e6),
+                       "parallelism": "replicas only (one independent call per GPU)" if world > 1 else "1 GPU"},
+            "ms_per_attention_call": round(kern_ms, 4),
+            "index_build_us": round(build_us, 1),
+            "pct_of_peak": {"measured_burst_%.1f" % pk["bf16_tflops"]: round(100 * achieved / pk["bf16_tflops"], 2),
+                            "measured_sustained_%.1f" % pk["bf16_tflops_sustained"]: round(100 * achieved / pk["bf16_tflops_sustained"], 2),
+                            "nominal_2250": round(100 * achieved / 2250.0, 2)},
+            "all_tiles": None if dense_ms is None else {
+                "ms": round(dense_ms, 3), "nnz": int(dense_nnz),
+                "speedup_lvsa_vs_all_tiles": round(dense_ms / kern_ms, 3),
+                "tflops": round(float(dense_nnz) * w.H * w.B * 4.0 * w.tile * w.tile * w.d / (dense_ms * 1e-3) / 1e12, 1)},
+            "roofline": {"bound": "tensor", "achieved": round(achieved, 2), "peak": peak,
+                         "unit": "TFLOP/s", "frac": round(achieved / peak, 4), "traffic": None,
+                         "peak_source": pk["_source"] + " bf16 burst (kernel timed alone, %d launches)" % ks,
+                         "kernel": "lvsa_attn_sm100", "flops_per_launch": kern_flops},
+            "cpu_baseline": cpu,
+            "e2e": None if e2e is None else {
+                "value": round(world * e2e["flops"] / (e2e["ms"] * 1e-3) / 1e12, 3), "unit": UNIT,
+                "ms_per_step": round(e2e["ms"], 3), "h2d_bytes_per_step": e2e["h2d"],
+                "d2h_bytes_per_step": e2e["d2h"]},
+            "gpu_launches": launches_per_step * args.steps,
+            "clocks": clocks,
+        }
+        print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def cpu_baseline(w, q, k, v, step, n_rows, nthreads=0):
+    """Times oracle O8 (fp64 Eq. 2) on a bounded sample of query rows of the same workload."""
+    from oracle import lvsa_oracle as orc
+    p = orc.pattern(w.T, w.W, w.a, step)
+    rows = inputs.sample_rows(w, n_uniform=n_rows, n_edge=0, seed=1)[:n_rows]
+    qa, ka, va = (inputs.to_oracle_array(x[0]) for x in (q, k, v))
+    t0 = time.perf_counter()
+    orc.attn_rows(qa, ka, va, w.T, w.P, p.A, rows, nthreads=nthreads)
+    sec = time.perf_counter() - t0
+    keys = sum(int(p.A[r // w.P].sum()) * w.P for r in rows)
+    flops = 4.0 * w.d * w.H * keys
+    cores = orc.num_threads() if nthreads == 0 else nthreads
+    return {"value": flops / sec / 1e12, "unit": "TFLOP/s (fp64, exact Eq. 2 flops)", "cores": cores,
+            "kind": "oracle", "seconds": round(sec, 2),
+            "sample": f"{len(rows)} seeded query rows x {w.H} heads of {w.name} at step {step}",
+            "extrapolated_ms_per_full_call": round(sec * 1e3 * w.N / len(rows), 1)}
+
+
+def run_reference(args):
+    """Reference arm = the oracle on the host cores; rank 0 only."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    w = inputs.WORKLOADS[args.workload]
+    q, k, v = inputs.make_qkv(w, "cpu", torch.bfloat16)
+    steps_cycle = list(w.steps) if w.steps else [0]
+    rows_per_step = args.cpu_rows
+    for i in range(args.warmup):
+        cpu_baseline(w, q, k, v, steps_cycle[i % len(steps_cycle)], max(1, rows_per_step // 8))
+    t0 = time.perf_counter()
+    fl, last = 0.0, None
+    for i in range(args.steps):
+        last = cpu_baseline(w, q, k, v, steps_cycle[i % len(steps_cycle)], rows_per_step)
+        fl += last["value"] * 1e12 * last["seconds"]
+    sec = time.perf_counter() - t0
+    val = fl / sec / 1e12
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": sec * 1e3 / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic (same seeded tensors as the CUDA arm)",
+            "config": {"workload": args.workload, "T": w.T, "P": w.P, "N": w.N, "H": w.H, "d": w.d},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": last["cores"], "kind": "oracle",
+                             "sample": f"each step: {last['sample']} (exact Eq. 2 flops, fp64)"},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="wan1.3b_6x", choices=sorted(inputs.WORKLOADS))
+    ap.add_argument("--cpu-rows", type=int, default=None, help="query rows in the oracle's timed sample")
+    ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-dense", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.cpu_rows is None:
+        # ~15 s of oracle time on 8 cores at the Wan 6x shape; scaled by heads
+        args.cpu_rows = max(16, int(768 * 12 / inputs.WORKLOADS[args.workload].H))
+        if args.impl == "reference":
+            args.cpu_rows = max(8, args.cpu_rows // 4)
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        if not torch.cuda.is_available():
+            raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()
