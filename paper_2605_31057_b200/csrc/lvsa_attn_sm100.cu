@@ -12,6 +12,8 @@
 #include <cuda.h>
 #include <cuda_bf16.h>
 
+#include <stdlib.h>
+
 #include "lvsa_internal.h"
 #include "sm100_ptx.cuh"
 
@@ -280,9 +282,11 @@ PFN_encodeTiled get_encode() {
     return fn;
 }
 
+}  // namespace
+
 // [B, N, H, d] bf16, d fastest.  Tensor-map dims (fastest first): d, H, N, B.  Box: 64 x 1 x rows x 1
 // with SWIZZLE_128B, i.e. smem tile [rows][128 B]; rows >= N are zero-filled.
-lvsa_status_t make_tmap(CUtensorMap *m, const void *base, long long N, int H, int d, int B, int box_rows) {
+lvsa_status_t lvsa_make_tmap_bf16(CUtensorMap *m, const void *base, long long N, int H, int d, int B, int box_rows) {
     PFN_encodeTiled enc = get_encode();
     if (enc == nullptr) { lvsa_set_error("cuTensorMapEncodeTiled entry point not found"); return LVSA_ECUDA; }
     cuuint64_t dims[4] = {(cuuint64_t)d, (cuuint64_t)H, (cuuint64_t)N, (cuuint64_t)B};
@@ -299,6 +303,8 @@ lvsa_status_t make_tmap(CUtensorMap *m, const void *base, long long N, int H, in
     return LVSA_OK;
 }
 
+namespace {
+
 float *g_dbg = nullptr;
 
 template <int D, int BT>
@@ -307,9 +313,9 @@ lvsa_status_t launch_v0(const lvsa_index *ix, const void *q, const void *k, cons
     using C = Cfg<D, BT>;
     CUtensorMap mq, mk, mv;
     lvsa_status_t st;
-    if ((st = make_tmap(&mq, q, ix->N, ix->p.H, D, ix->p.B, 128)) != LVSA_OK) return st;
-    if ((st = make_tmap(&mk, k, ix->N, ix->p.H, D, ix->p.B, BT)) != LVSA_OK) return st;
-    if ((st = make_tmap(&mv, v, ix->N, ix->p.H, D, ix->p.B, BT)) != LVSA_OK) return st;
+    if ((st = lvsa_make_tmap_bf16(&mq, q, ix->N, ix->p.H, D, ix->p.B, 128)) != LVSA_OK) return st;
+    if ((st = lvsa_make_tmap_bf16(&mk, k, ix->N, ix->p.H, D, ix->p.B, BT)) != LVSA_OK) return st;
+    if ((st = lvsa_make_tmap_bf16(&mv, v, ix->N, ix->p.H, D, ix->p.B, BT)) != LVSA_OK) return st;
     auto kern = lvsa_attn_sm100_v0_kernel<D, BT>;
     LVSA_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
     const float scale_log2 = ix->p.softmax_scale * 1.4426950408889634f;
@@ -338,6 +344,11 @@ lvsa_status_t lvsa_attn_sm100_launch(const lvsa_index *ix, const void *q, const 
         lvsa_set_error("tcgen05 kernel: H and B must be <= 65535");
         return LVSA_EUNSUPPORTED;
     }
-    if (ix->p.d == 128) return launch_v0<128, 128>(ix, q, k, v, out, lse, stream);
+    if (ix->p.d == 128) {
+        // LVSA_SM100_V0=1 selects the bring-up kernel (debugging aid; same results)
+        static const bool force_v0 = getenv("LVSA_SM100_V0") != nullptr && getenv("LVSA_SM100_V0")[0] == '1';
+        if (force_v0 || g_dbg != nullptr) return launch_v0<128, 128>(ix, q, k, v, out, lse, stream);
+        return lvsa_attn_sm100_ws_launch(ix, q, k, v, out, lse, stream);
+    }
     return launch_v0<64, 64>(ix, q, k, v, out, lse, stream);
 }

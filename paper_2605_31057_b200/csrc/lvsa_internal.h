@@ -60,3 +60,7 @@ lvsa_status_t lvsa_attn_simt_launch(const lvsa_index *ix, const void *q, const v
 lvsa_status_t lvsa_attn_sm100_launch(const lvsa_index *ix, const void *q, const void *k,
                                      const void *v, void *out, float *lse, cudaStream_t stream);
 int lvsa_attn_sm100_supported(const lvsa_index *ix);
+
+// lvsa_attn_sm100_ws.cu (warp-specialised persistent kernel, d = 128)
+lvsa_status_t lvsa_attn_sm100_ws_launch(const lvsa_index *ix, const void *q, const void *k,
+                                        const void *v, void *out, float *lse, cudaStream_t stream);
