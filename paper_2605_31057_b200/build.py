@@ -29,6 +29,9 @@ def stale() -> bool:
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
+    override = os.environ.get("LVSA_LIB")   # a prebuilt liblvsa.so (e.g. a tuning variant)
+    if override and not force:
+        return override
     if not force and not stale():
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")

@@ -16,6 +16,7 @@
 
 #include "lvsa_internal.h"
 #include "sm100_ptx.cuh"
+#include "lvsa_softmax.cuh"
 
 using namespace sm100;
 
@@ -26,6 +27,9 @@ constexpr int TILE_BYTES = BT * D * 2;          // 32 KB: one Q, K or V tile
 constexpr int HALF_BYTES = BT * 128;            // 16 KB: [128 rows][128 B] swizzle span
 constexpr int NTHREADS = 384;
 constexpr float RESCALE_THRESHOLD = 8.0f;       // log2 units: rescale O only if the max grew by > 2^8
+#ifndef LVSA_POLY_PAIRS
+#define LVSA_POLY_PAIRS 0                       // of every 16 logit pairs, how many take the FMA-pipe exp2
+#endif
 
 template <int NS>
 struct Smem {
@@ -34,8 +38,8 @@ struct Smem {
     static constexpr int BAR_OFF = RING_OFF + NS * TILE_BYTES;
     // barriers (8 B each)
     static constexpr int Q_FULL = 0, Q_EMPTY = 1, S_FULL = 2 /*2*/, P_FULL = 4 /*2*/, O_FULL = 6 /*2*/,
-                         O_FREE = 8 /*2*/, KV_FULL = 10 /*NS*/, KV_EMPTY = 10 + NS /*NS*/,
-                         NBARS = 10 + 2 * NS;
+                         O_FREE = 8 /*2*/, P2_FULL = 10 /*2*/, KV_FULL = 12 /*NS*/, KV_EMPTY = 12 + NS /*NS*/,
+                         NBARS = 12 + 2 * NS;
     static constexpr int TMEM_SLOT_OFF = BAR_OFF + 8 * NBARS;
     static constexpr int BYTES = TMEM_SLOT_OFF + 16 + 1024 /*alignment slack*/;
 };
@@ -75,6 +79,7 @@ lvsa_attn_sm100_ws_kernel(const __grid_constant__ CUtensorMap tmap_q,
         mbar_init(bar(SM::Q_FULL), 1); mbar_init(bar(SM::Q_EMPTY), 1);
         for (int w = 0; w < 2; ++w) {
             mbar_init(bar(SM::S_FULL + w), 1); mbar_init(bar(SM::P_FULL + w), 4);
+            mbar_init(bar(SM::P2_FULL + w), 4);
             mbar_init(bar(SM::O_FULL + w), 1); mbar_init(bar(SM::O_FREE + w), 4);
         }
         for (int s = 0; s < NS; ++s) { mbar_init(bar(SM::KV_FULL + s), 1); mbar_init(bar(SM::KV_EMPTY + s), 1); }
@@ -140,13 +145,7 @@ lvsa_attn_sm100_ws_kernel(const __grid_constant__ CUtensorMap tmap_q,
                         if (!((cm[c >> 5] >> (c & 31)) & 1u)) s[c] = -INFINITY;
                 }
 
-                float mx0 = s[0], mx1 = s[1], mx2 = s[2], mx3 = s[3];
-#pragma unroll
-                for (int c = 4; c < BT; c += 4) {
-                    mx0 = fmaxf(mx0, s[c]); mx1 = fmaxf(mx1, s[c + 1]);
-                    mx2 = fmaxf(mx2, s[c + 2]); mx3 = fmaxf(mx3, s[c + 3]);
-                }
-                const float rm = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)) * scale_log2;
+                const float rm = lvsa_sm::row_max<BT>(s) * scale_log2;
                 if (cnt == 0) {
                     m_run = rm;
                 } else {
@@ -168,24 +167,41 @@ lvsa_attn_sm100_ws_kernel(const __grid_constant__ CUtensorMap tmap_q,
                     }
                 }
                 const float m_use = (m_run == -INFINITY) ? 0.f : m_run;
-                float ls0 = 0.f, ls1 = 0.f;
+                // P = exp2(S * scale - m) as bf16 over S's first 64 columns, published in two
+                // halves so that the first four k-blocks of O += P V can start while the second
+                // half of the exponentials is still being computed.
+                const uint64_t scale2 = lvsa_sm::pack2(scale_log2, scale_log2);
+                const uint64_t negm2 = lvsa_sm::pack2(-m_use, -m_use);
+                uint64_t lsum = lvsa_sm::pack2(0.f, 0.f);
+                auto publish = [&](int which) {
+                    tmem_wait_st();
+                    tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(bar(which + w));
+                };
+                if (st == LVSA_ST_FULL) {
 #pragma unroll
-                for (int c = 0; c < 4; ++c) {
-                    uint32_t pk[16];
-#pragma unroll
-                    for (int x = 0; x < 16; ++x) {
-                        const float p0 = fast_exp2(fmaf(s[c * 32 + 2 * x], scale_log2, -m_use));
-                        const float p1 = fast_exp2(fmaf(s[c * 32 + 2 * x + 1], scale_log2, -m_use));
-                        ls0 += p0; ls1 += p1;
-                        pk[x] = pack_bf16x2(p0, p1);
+                    for (int c = 0; c < 4; ++c) {
+                        uint32_t pk[16];
+                        lvsa_sm::exp_chunk32<LVSA_POLY_PAIRS>(s, c * 32, scale2, negm2, pk, lsum);
+                        tmem_st_32x32b_x16(tS + c * 16, pk);
+                        if (c == 1) publish(SM::P_FULL);
                     }
-                    tmem_st_32x32b_x16(tS + c * 16, pk);
+                } else {   // masked logits are -inf: the MUFU path gives exact zeros
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) {
+                        uint32_t pk[16];
+                        lvsa_sm::exp_chunk32<0>(s, c * 32, scale2, negm2, pk, lsum);
+                        tmem_st_32x32b_x16(tS + c * 16, pk);
+                        if (c == 1) publish(SM::P_FULL);
+                    }
                 }
-                l_run += ls0 + ls1;
-                tmem_wait_st();
-                tc_fence_before();
-                __syncwarp();
-                if (lane == 0) mbar_arrive(bar(SM::P_FULL + w));
+                publish(SM::P2_FULL);
+                {
+                    float la, lb;
+                    lvsa_sm::unpack2(lsum, la, lb);
+                    l_run += la + lb;
+                }
                 ++cnt;
             }
             if (cnt > 0) {
@@ -254,8 +270,11 @@ lvsa_attn_sm100_ws_kernel(const __grid_constant__ CUtensorMap tmap_q,
                     }
                 }
             }
-        } else if (warp == 9 && lane == 0) {
+        } else if (warp == 9) {
             // =========================================================== MMA issuer
+            // The whole warp runs the control flow (waits included); one elected lane issues.
+            // Under elect.sync the compiler keeps descriptors in uniform registers with no
+            // per-lane waterfall around every tcgen05.mma.
             constexpr uint32_t IDESC_S = umma_idesc_bf16(128, BT, 0);
             constexpr uint32_t IDESC_O = umma_idesc_bf16(128, D, 1);
             const uint64_t dQ = umma_smem_desc_sw128(sQ, 16);
@@ -270,9 +289,9 @@ lvsa_attn_sm100_ws_kernel(const __grid_constant__ CUtensorMap tmap_q,
                 }
                 umma_commit(bar(SM::S_FULL + w));
             };
-            auto issue_PV = [&](int w, uint32_t stageV, bool accumulate) {
+            auto issue_PV = [&](int w, uint32_t stageV, bool accumulate, int half) {
 #pragma unroll
-                for (int kk = 0; kk < 8; ++kk)
+                for (int kk = 4 * half; kk < 4 * half + 4; ++kk)
                     umma_ts(tmem_base + 256 + w * 128, tmem_base + w * 128 + kk * 8,
                             dRingV + (uint64_t)(((stageV * TILE_BYTES) >> 4) + ((kk * 2048) >> 4)), IDESC_O,
                             (accumulate || kk > 0) ? 1u : 0u);
@@ -280,56 +299,73 @@ lvsa_attn_sm100_ws_kernel(const __grid_constant__ CUtensorMap tmap_q,
             uint32_t kv_it = 0, qi = 0, pc[2] = {0, 0}, oc[2] = {0, 0};
             for (long long work = blockIdx.x; work < n_work; work += gridDim.x) {
                 const int item = (int)(work % n_items);
-                const int e0 = item_ptr[item], e1 = item_ptr[item + 1];
+                const int e0 = __shfl_sync(0xffffffffu, __ldg(item_ptr + item), 0);
+                const int e1 = __shfl_sync(0xffffffffu, __ldg(item_ptr + item + 1), 0);
                 if (e0 == e1) continue;   // cannot happen (t in A(t)), kept for symmetry with the producer
                 bool started[2] = {false, false};
                 mbar_wait(bar(SM::Q_FULL), qi & 1u); ++qi;
-                int entry = __ldg(item_tiles + e0);
+                int entry = __shfl_sync(0xffffffffu, __ldg(item_tiles + e0), 0);
                 {   // S(0) for both q tiles
                     const uint32_t stageK = kv_it % NS, n = kv_it / NS;
                     mbar_wait(bar(SM::KV_FULL + stageK), n & 1u);
                     tc_fence_after();
+                    if (elect_one_sync()) {
 #pragma unroll
-                    for (int w = 0; w < 2; ++w)
-                        if (entry_state(entry, w) != LVSA_ST_SKIP) issue_S(w, stageK);
-                    umma_commit(bar(SM::KV_EMPTY + stageK));
+                        for (int w = 0; w < 2; ++w)
+                            if (entry_state(entry, w) != LVSA_ST_SKIP) issue_S(w, stageK);
+                        umma_commit(bar(SM::KV_EMPTY + stageK));
+                    }
+                    __syncwarp();
                     ++kv_it;
                 }
                 for (int e = e0; e < e1; ++e) {
                     const bool has_next = e + 1 < e1;
-                    const int entry_n = has_next ? __ldg(item_tiles + e + 1) : 0;
+                    const int entry_n = has_next ? __shfl_sync(0xffffffffu, __ldg(item_tiles + e + 1), 0) : 0;
                     const uint32_t stageV = kv_it % NS, nV = kv_it / NS;
                     ++kv_it;
                     uint32_t stageK = 0, nK = 0;
                     if (has_next) { stageK = kv_it % NS; nK = kv_it / NS; ++kv_it; }
                     mbar_wait(bar(SM::KV_FULL + stageV), nV & 1u);
-                    bool k_ready = false;
+                    if (has_next) mbar_wait(bar(SM::KV_FULL + stageK), nK & 1u);
                     // Q is last read by the S MMAs of the final tile, all issued by now
-                    if (!has_next) umma_commit(bar(SM::Q_EMPTY));
+                    if (!has_next && elect_one_sync()) umma_commit(bar(SM::Q_EMPTY));
 #pragma unroll
                     for (int w = 0; w < 2; ++w) {
-                        if (entry_state(entry, w) != LVSA_ST_SKIP) {
+                        const bool do_pv = entry_state(entry, w) != LVSA_ST_SKIP;
+                        const bool do_s = has_next && entry_state(entry_n, w) != LVSA_ST_SKIP;
+                        if (do_pv) {
                             if (!started[w]) mbar_wait(bar(SM::O_FREE + w), (oc[w] & 1u) ^ 1u);
                             mbar_wait(bar(SM::P_FULL + w), pc[w] & 1u); ++pc[w];
+                        }
+                        tc_fence_after();
+                        if (do_pv) {
+                            if (elect_one_sync()) issue_PV(w, stageV, started[w], 0);
+                            __syncwarp();
+                            mbar_wait(bar(SM::P2_FULL + w), (pc[w] & 1u) ^ 1u);   // pc already advanced
                             tc_fence_after();
-                            issue_PV(w, stageV, started[w]);
-                            started[w] = true;
                         }
-                        if (has_next && entry_state(entry_n, w) != LVSA_ST_SKIP) {
-                            if (!k_ready) { mbar_wait(bar(SM::KV_FULL + stageK), nK & 1u); tc_fence_after(); k_ready = true; }
-                            issue_S(w, stageK);
+                        if (elect_one_sync()) {
+                            if (do_pv) issue_PV(w, stageV, started[w], 1);
+                            if (do_s) issue_S(w, stageK);
                         }
+                        __syncwarp();
+                        started[w] |= do_pv;
                     }
-                    umma_commit(bar(SM::KV_EMPTY + stageV));
-                    if (has_next) {
-                        if (!k_ready) mbar_wait(bar(SM::KV_FULL + stageK), nK & 1u);   // keep ring parity in step
-                        umma_commit(bar(SM::KV_EMPTY + stageK));
+                    if (elect_one_sync()) {
+                        umma_commit(bar(SM::KV_EMPTY + stageV));
+                        if (has_next) umma_commit(bar(SM::KV_EMPTY + stageK));
                     }
+                    __syncwarp();
                     entry = entry_n;
                 }
+                if (elect_one_sync()) {
 #pragma unroll
-                for (int w = 0; w < 2; ++w)
-                    if (started[w]) { umma_commit(bar(SM::O_FULL + w)); ++oc[w]; }
+                    for (int w = 0; w < 2; ++w)
+                        if (started[w]) umma_commit(bar(SM::O_FULL + w));
+                }
+                __syncwarp();
+#pragma unroll
+                for (int w = 0; w < 2; ++w) if (started[w]) ++oc[w];
             }
         }
     }
