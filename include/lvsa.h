@@ -86,8 +86,12 @@ typedef struct lvsa_index_info {
  *   indptr[nq+1], indices[nnz] ascending within a q tile, flags[nnz] in {FULL, PARTIAL}.
  * A kv tile is kept iff some (valid query row, valid key column) pair is allowed; it is PARTIAL
  * iff some (valid row, column of the tile) pair is not (frame not attended, or column >= N).
- * All arithmetic is integer and runs in CUDA kernels on the current device's default stream;
- * the call synchronises once to learn nnz.  Returns NULL on error (lvsa_last_error()).
+ * All arithmetic is integer and runs in CUDA kernels on the current device's default stream.
+ * The call only ENQUEUES the seven builder kernels and returns: it never synchronises.  Device
+ * buffers come from one stream-ordered allocation sized by an upper bound on nnz (no device
+ * round trip); the counters (nnz, ...) are read back lazily by lvsa_index_info /
+ * lvsa_index_copy_host, which do synchronise.  Use the index on the stream it was built on (or
+ * order other streams after it).  Returns NULL on error (lvsa_last_error()).
  * The handle is owned by the library; free it with lvsa_index_destroy.  It is immutable and
  * may be used by any number of lvsa_attn_fwd calls.
  */
@@ -117,13 +121,22 @@ lvsa_status_t lvsa_attn_fwd(const void *q, const void *k, const void *v,
 
 /*
  * lvsa_attn_fwd_host — the same call for HOST buffers (pinned or pageable): copies q, k, v to
- * device scratch owned by the index (allocated on first use), runs lvsa_attn_fwd on `stream`,
- * copies out (and lse if not NULL) back, and synchronises `stream` before returning.
+ * a device workspace owned by the library (one per process, allocated on first use, grown on
+ * demand, shared by all indices; freed by lvsa_workspace_release), runs lvsa_attn_fwd on
+ * `stream`, copies out (and lse if not NULL) back, and synchronises `stream` before returning.
+ * Calls through the workspace are serialised by a mutex.
  */
 lvsa_status_t lvsa_attn_fwd_host(const void *q_host, const void *k_host, const void *v_host,
                                  lvsa_index_t *index, void *out_host, float *lse_host,
                                  void *stream);
 
+/* Frees the device workspace of lvsa_attn_fwd_host (synchronises the device).  Safe to call
+ * at any time when no lvsa_attn_fwd_host call is in flight; the next host call re-allocates. */
+void lvsa_workspace_release(void);
+
+/* Frees the index.  Its device buffers are stream-ordered memory: they are released behind the
+ * work already enqueued on the stream that last used the index, without synchronising (if the
+ * index was used on more than one stream the device is synchronised first). */
 void lvsa_index_destroy(lvsa_index_t *index);
 
 lvsa_status_t lvsa_index_info(const lvsa_index_t *index, lvsa_index_info_t *info);

@@ -45,7 +45,7 @@ class IndexInfo(C.Structure):
 
 EXPORTS = ("lvsa_build_block_index", "lvsa_build_block_index_ex", "lvsa_attn_fwd",
            "lvsa_attn_fwd_host", "lvsa_index_destroy", "lvsa_index_info", "lvsa_index_copy_host",
-           "lvsa_attn_fwd_launches", "lvsa_last_error", "lvsa_version")
+           "lvsa_attn_fwd_launches", "lvsa_workspace_release", "lvsa_last_error", "lvsa_version")
 
 _lib = None
 

@@ -6,7 +6,8 @@
 //   warps 0-3  softmax warpgroup 0 : rows of q tile 0   (TMEM lanes = rows; thread = one row)
 //   warps 4-7  softmax warpgroup 1 : rows of q tile 1
 //   warp  8    TMA producer        : Q once per item, then K_j, V_j of each listed tile into a ring
-//   warp  9    MMA issuer          : S_w = Q_w K_j^T and O_w += P_w V_j (tcgen05, TMEM accumulators)
+//   warps 9,10 MMA issuers         : S_w = Q_w K_j^T and O_w += P_w V_j (tcgen05, TMEM accumulators),
+//                                    warp 9 for q tile 0, warp 10 for q tile 1
 // TMEM (512 columns): S0 [0,128) S1 [128,256) O0 [256,384) O1 [384,512); P_w (bf16) overwrites the
 // first 64 columns of S_w and is the A operand of the second MMA straight from TMEM.
 // The tensor pipe executes MMAs in issue order, which is what makes the S/P aliasing and the
@@ -38,8 +39,8 @@ struct Smem {
     static constexpr int BAR_OFF = RING_OFF + NS * TILE_BYTES;
     // barriers (8 B each)
     static constexpr int Q_FULL = 0, Q_EMPTY = 1, S_FULL = 2 /*2*/, P_FULL = 4 /*2*/, O_FULL = 6 /*2*/,
-                         O_FREE = 8 /*2*/, P2_FULL = 10 /*2*/, KV_FULL = 12 /*NS*/, KV_EMPTY = 12 + NS /*NS*/,
-                         NBARS = 12 + 2 * NS;
+                         O_FREE = 8 /*2*/, P2_FULL = 10 /*2*/, TURN = 12 /*2*/, KV_FULL = 14 /*NS*/, KV_EMPTY = 14 + NS /*NS*/,
+                         NBARS = 14 + 2 * NS;
     static constexpr int TMEM_SLOT_OFF = BAR_OFF + 8 * NBARS;
     static constexpr int BYTES = TMEM_SLOT_OFF + 16 + 1024 /*alignment slack*/;
 };
@@ -76,13 +77,14 @@ lvsa_attn_sm100_ws_kernel(const __grid_constant__ CUtensorMap tmap_q,
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, wg = tid >> 7;
 
     if (warp == 8 && lane == 0) {
-        mbar_init(bar(SM::Q_FULL), 1); mbar_init(bar(SM::Q_EMPTY), 1);
+        mbar_init(bar(SM::Q_FULL), 1); mbar_init(bar(SM::Q_EMPTY), 2);
         for (int w = 0; w < 2; ++w) {
             mbar_init(bar(SM::S_FULL + w), 1); mbar_init(bar(SM::P_FULL + w), 4);
             mbar_init(bar(SM::P2_FULL + w), 4);
             mbar_init(bar(SM::O_FULL + w), 1); mbar_init(bar(SM::O_FREE + w), 4);
+            mbar_init(bar(SM::TURN + w), 1);
         }
-        for (int s = 0; s < NS; ++s) { mbar_init(bar(SM::KV_FULL + s), 1); mbar_init(bar(SM::KV_EMPTY + s), 1); }
+        for (int s = 0; s < NS; ++s) { mbar_init(bar(SM::KV_FULL + s), 1); mbar_init(bar(SM::KV_EMPTY + s), 2); }
         fence_barrier_init();
         prefetch_tmap(&tmap_q); prefetch_tmap(&tmap_k); prefetch_tmap(&tmap_v);
     }
@@ -119,6 +121,12 @@ lvsa_attn_sm100_ws_kernel(const __grid_constant__ CUtensorMap tmap_q,
 
                 mbar_wait(bar(SM::S_FULL + w), sc & 1u); ++sc;
                 tc_fence_after();
+#ifdef LVSA_DIAG_NOSOFTMAX   // timing diagnostic only (wrong results): MMA/TMA pipeline alone
+                tc_fence_before(); __syncwarp();
+                if (lane == 0) { mbar_arrive(bar(SM::P_FULL + w)); mbar_arrive(bar(SM::P2_FULL + w)); }
+                ++cnt; l_run = 1.f; m_run = 0.f;
+                continue;
+#endif
                 float s[BT];
 #pragma unroll
                 for (int c = 0; c < 4; ++c) {
@@ -270,49 +278,53 @@ lvsa_attn_sm100_ws_kernel(const __grid_constant__ CUtensorMap tmap_q,
                     }
                 }
             }
-        } else if (warp == 9) {
-            // =========================================================== MMA issuer
+        } else if (warp == 9 || warp == 10) {
+            // =========================================================== MMA issuers
+            // One issuing warp per q tile (w = 0: warp 9, w = 1: warp 10).  A single warp issuing all
+            // 32 MMAs of a kv tile plus their descriptor moves was itself the limiter (measured with
+            // the softmax disabled: tensor pipe 73 % busy, issuer never idle).  The two chains
+            // softmax_w -> PV_w -> S_w are independent; they only share the K/V ring and Q, whose
+            // "empty" barriers therefore take one commit from each issuer.
             // The whole warp runs the control flow (waits included); one elected lane issues.
             // Under elect.sync the compiler keeps descriptors in uniform registers with no
             // per-lane waterfall around every tcgen05.mma.
+            const int w = warp - 9;
             constexpr uint32_t IDESC_S = umma_idesc_bf16(128, BT, 0);
             constexpr uint32_t IDESC_O = umma_idesc_bf16(128, D, 1);
-            const uint64_t dQ = umma_smem_desc_sw128(sQ, 16);
+            const uint64_t dQ = umma_smem_desc_sw128(sQ + w * TILE_BYTES, 16);
             const uint64_t dRingK = umma_smem_desc_sw128(sRing, 16);
             const uint64_t dRingV = umma_smem_desc_sw128(sRing, HALF_BYTES);
-            auto issue_S = [&](int w, uint32_t stageK) {
+            const uint32_t tS = tmem_base + w * 128, tO = tmem_base + 256 + w * 128;
+            auto issue_S = [&](uint32_t stageK) {
 #pragma unroll
                 for (int kk = 0; kk < 8; ++kk) {
                     const uint32_t off = (uint32_t)((kk >> 2) * HALF_BYTES + (kk & 3) * 32) >> 4;
-                    umma_ss(tmem_base + w * 128, dQ + (uint64_t)(((uint32_t)(w * TILE_BYTES) >> 4) + off),
-                            dRingK + (uint64_t)(((stageK * TILE_BYTES) >> 4) + off), IDESC_S, kk > 0);
+                    umma_ss(tS, dQ + (uint64_t)off, dRingK + (uint64_t)(((stageK * TILE_BYTES) >> 4) + off),
+                            IDESC_S, kk > 0);
                 }
                 umma_commit(bar(SM::S_FULL + w));
             };
-            auto issue_PV = [&](int w, uint32_t stageV, bool accumulate, int half) {
+            auto issue_PV = [&](uint32_t stageV, bool accumulate, int half) {
 #pragma unroll
                 for (int kk = 4 * half; kk < 4 * half + 4; ++kk)
-                    umma_ts(tmem_base + 256 + w * 128, tmem_base + w * 128 + kk * 8,
-                            dRingV + (uint64_t)(((stageV * TILE_BYTES) >> 4) + ((kk * 2048) >> 4)), IDESC_O,
-                            (accumulate || kk > 0) ? 1u : 0u);
+                    umma_ts(tO, tS + kk * 8, dRingV + (uint64_t)(((stageV * TILE_BYTES) >> 4) + ((kk * 2048) >> 4)),
+                            IDESC_O, (accumulate || kk > 0) ? 1u : 0u);
             };
-            uint32_t kv_it = 0, qi = 0, pc[2] = {0, 0}, oc[2] = {0, 0};
+            uint32_t kv_it = 0, qi = 0, pc = 0, oc = 0, turn = 0;
             for (long long work = blockIdx.x; work < n_work; work += gridDim.x) {
                 const int item = (int)(work % n_items);
                 const int e0 = __shfl_sync(0xffffffffu, __ldg(item_ptr + item), 0);
                 const int e1 = __shfl_sync(0xffffffffu, __ldg(item_ptr + item + 1), 0);
                 if (e0 == e1) continue;   // cannot happen (t in A(t)), kept for symmetry with the producer
-                bool started[2] = {false, false};
+                bool started = false;
                 mbar_wait(bar(SM::Q_FULL), qi & 1u); ++qi;
                 int entry = __shfl_sync(0xffffffffu, __ldg(item_tiles + e0), 0);
-                {   // S(0) for both q tiles
+                {   // S(0)
                     const uint32_t stageK = kv_it % NS, n = kv_it / NS;
                     mbar_wait(bar(SM::KV_FULL + stageK), n & 1u);
                     tc_fence_after();
                     if (elect_one_sync()) {
-#pragma unroll
-                        for (int w = 0; w < 2; ++w)
-                            if (entry_state(entry, w) != LVSA_ST_SKIP) issue_S(w, stageK);
+                        if (entry_state(entry, w) != LVSA_ST_SKIP) issue_S(stageK);
                         umma_commit(bar(SM::KV_EMPTY + stageK));
                     }
                     __syncwarp();
@@ -325,47 +337,55 @@ lvsa_attn_sm100_ws_kernel(const __grid_constant__ CUtensorMap tmap_q,
                     ++kv_it;
                     uint32_t stageK = 0, nK = 0;
                     if (has_next) { stageK = kv_it % NS; nK = kv_it / NS; ++kv_it; }
-                    mbar_wait(bar(SM::KV_FULL + stageV), nV & 1u);
-                    if (has_next) mbar_wait(bar(SM::KV_FULL + stageK), nK & 1u);
-                    // Q is last read by the S MMAs of the final tile, all issued by now
+                    const bool do_pv = entry_state(entry, w) != LVSA_ST_SKIP;
+                    const bool do_s = has_next && entry_state(entry_n, w) != LVSA_ST_SKIP;
+                    // Q_w is last read by the S MMAs of the final tile, all issued by now
                     if (!has_next && elect_one_sync()) umma_commit(bar(SM::Q_EMPTY));
-#pragma unroll
-                    for (int w = 0; w < 2; ++w) {
-                        const bool do_pv = entry_state(entry, w) != LVSA_ST_SKIP;
-                        const bool do_s = has_next && entry_state(entry_n, w) != LVSA_ST_SKIP;
-                        if (do_pv) {
-                            if (!started[w]) mbar_wait(bar(SM::O_FREE + w), (oc[w] & 1u) ^ 1u);
-                            mbar_wait(bar(SM::P_FULL + w), pc[w] & 1u); ++pc[w];
-                        }
+                    __syncwarp();
+                    // Both issuers wait for every stage, used or not: a stage's KV_EMPTY takes one
+                    // commit from each, so neither may run a whole ring ahead of the other.
+                    mbar_wait(bar(SM::KV_FULL + stageV), nV & 1u);
+#ifndef LVSA_NO_TURNS
+                    // The issuers take turns, q tile 0 first: that keeps the two softmax warpgroups
+                    // half a period apart, so each has the MUFU to itself while the tensor pipe
+                    // works for the other (left to themselves the two chains fall into step and the
+                    // exponentials of both q tiles collide: measured 40 ms instead of 35 ms).
+                    mbar_wait(bar(SM::TURN + w), (turn & 1u) ^ (w == 0 ? 1u : 0u));
+                    ++turn;
+#endif
+                    if (do_pv) {
+                        if (!started) mbar_wait(bar(SM::O_FREE + w), (oc & 1u) ^ 1u);
+                        mbar_wait(bar(SM::P_FULL + w), pc & 1u);
                         tc_fence_after();
-                        if (do_pv) {
-                            if (elect_one_sync()) issue_PV(w, stageV, started[w], 0);
-                            __syncwarp();
-                            mbar_wait(bar(SM::P2_FULL + w), (pc[w] & 1u) ^ 1u);   // pc already advanced
-                            tc_fence_after();
-                        }
-                        if (elect_one_sync()) {
-                            if (do_pv) issue_PV(w, stageV, started[w], 1);
-                            if (do_s) issue_S(w, stageK);
-                        }
+                        if (elect_one_sync()) issue_PV(stageV, started, 0);
                         __syncwarp();
-                        started[w] |= do_pv;
+                        mbar_wait(bar(SM::P2_FULL + w), pc & 1u);
+                        ++pc;
+                        tc_fence_after();
+                    }
+                    if (has_next) {
+                        mbar_wait(bar(SM::KV_FULL + stageK), nK & 1u);
+                        tc_fence_after();
                     }
                     if (elect_one_sync()) {
+                        if (do_pv) issue_PV(stageV, started, 1);
+                        if (do_s) issue_S(stageK);
+                        // a stage this issuer never read (skipped q tile) is released at once
                         umma_commit(bar(SM::KV_EMPTY + stageV));
                         if (has_next) umma_commit(bar(SM::KV_EMPTY + stageK));
+#ifndef LVSA_NO_TURNS
+                        mbar_arrive(bar(SM::TURN + (w ^ 1)));
+#endif
                     }
                     __syncwarp();
+                    started |= do_pv;
                     entry = entry_n;
                 }
-                if (elect_one_sync()) {
-#pragma unroll
-                    for (int w = 0; w < 2; ++w)
-                        if (started[w]) umma_commit(bar(SM::O_FULL + w));
+                if (started) {
+                    if (elect_one_sync()) umma_commit(bar(SM::O_FULL + w));
+                    __syncwarp();
+                    ++oc;
                 }
-                __syncwarp();
-#pragma unroll
-                for (int w = 0; w < 2; ++w) if (started[w]) ++oc[w];
             }
         }
     }

@@ -2,6 +2,7 @@
 #include <math.h>
 #include <string.h>
 
+#include <mutex>
 #include <new>
 
 #include "lvsa_internal.h"
@@ -14,6 +15,10 @@ lvsa_status_t lvsa_cuda_fail(cudaError_t e, const char *what) {
     g_last_error = std::string(what) + ": " + cudaGetErrorName(e) + " (" + cudaGetErrorString(e) + ")";
     return LVSA_ECUDA;
 }
+
+// staging buffers of lvsa_attn_fwd_host (process-wide, one device at a time)
+static struct { void *ptr = nullptr; size_t cap = 0; int device = -1; } g_ws;
+static std::mutex g_ws_mutex;
 
 static size_t elem_size(const lvsa_index *ix) { return ix->p.dtype == LVSA_DTYPE_FP32 ? 4 : 2; }
 
@@ -107,6 +112,11 @@ lvsa_status_t lvsa_attn_fwd(const void *q, const void *k, const void *v, const l
         lvsa_set_error("q, k, v, out must be 16-byte aligned");
         return LVSA_EINVAL;
     }
+    if (index->last_stream != (cudaStream_t)stream) {
+        // the arena is stream-ordered memory: remember when it is no longer owned by one stream
+        index->multi_stream = true;
+        index->last_stream = (cudaStream_t)stream;
+    }
     if (use_tcgen05(index)) return lvsa_attn_sm100_launch(index, q, k, v, out, lse, (cudaStream_t)stream);
     return lvsa_attn_simt_launch(index, q, k, v, out, lse, (cudaStream_t)stream);
 }
@@ -120,36 +130,52 @@ lvsa_status_t lvsa_attn_fwd_host(const void *qh, const void *kh, const void *vh,
     cudaStream_t stream = (cudaStream_t)stream_;
     const size_t bytes = (size_t)ix->p.B * ix->N * ix->p.H * ix->p.d * elem_size(ix);
     const size_t lbytes = sizeof(float) * (size_t)ix->p.B * ix->p.H * ix->N;
-    if (ix->s_q == nullptr) {
-        LVSA_CUDA_TRY(cudaMalloc(&ix->s_q, bytes));
-        LVSA_CUDA_TRY(cudaMalloc(&ix->s_k, bytes));
-        LVSA_CUDA_TRY(cudaMalloc(&ix->s_v, bytes));
-        LVSA_CUDA_TRY(cudaMalloc(&ix->s_o, bytes));
-        LVSA_CUDA_TRY(cudaMalloc(&ix->s_lse, lbytes));
+    // device staging buffers: one process-wide workspace per device, grown on demand, shared by
+    // every index handle (a per-step rebuild of the index must not re-allocate gigabytes)
+    const size_t ab = (bytes + 255) & ~(size_t)255;
+    const size_t need = 4 * ab + lbytes;
+    std::lock_guard<std::mutex> lock(g_ws_mutex);
+    if (g_ws.ptr == nullptr || g_ws.cap < need || g_ws.device != ix->device) {
+        if (g_ws.ptr != nullptr) { cudaFree(g_ws.ptr); g_ws.ptr = nullptr; g_ws.cap = 0; }
+        LVSA_CUDA_TRY(cudaMalloc(&g_ws.ptr, need));
+        g_ws.cap = need; g_ws.device = ix->device;
     }
-    LVSA_CUDA_TRY(cudaMemcpyAsync(ix->s_q, qh, bytes, cudaMemcpyHostToDevice, stream));
-    LVSA_CUDA_TRY(cudaMemcpyAsync(ix->s_k, kh, bytes, cudaMemcpyHostToDevice, stream));
-    LVSA_CUDA_TRY(cudaMemcpyAsync(ix->s_v, vh, bytes, cudaMemcpyHostToDevice, stream));
-    lvsa_status_t st = lvsa_attn_fwd(ix->s_q, ix->s_k, ix->s_v, ix, ix->s_o, ix->s_lse, stream);
+    uint8_t *wsp = static_cast<uint8_t *>(g_ws.ptr);
+    void *s_q = wsp, *s_k = wsp + ab, *s_v = wsp + 2 * ab, *s_o = wsp + 3 * ab;
+    float *s_lse = reinterpret_cast<float *>(wsp + 4 * ab);
+    LVSA_CUDA_TRY(cudaMemcpyAsync(s_q, qh, bytes, cudaMemcpyHostToDevice, stream));
+    LVSA_CUDA_TRY(cudaMemcpyAsync(s_k, kh, bytes, cudaMemcpyHostToDevice, stream));
+    LVSA_CUDA_TRY(cudaMemcpyAsync(s_v, vh, bytes, cudaMemcpyHostToDevice, stream));
+    lvsa_status_t st = lvsa_attn_fwd(s_q, s_k, s_v, ix, s_o, s_lse, stream);
     if (st != LVSA_OK) return st;
-    LVSA_CUDA_TRY(cudaMemcpyAsync(oh, ix->s_o, bytes, cudaMemcpyDeviceToHost, stream));
-    if (lseh != nullptr) LVSA_CUDA_TRY(cudaMemcpyAsync(lseh, ix->s_lse, lbytes, cudaMemcpyDeviceToHost, stream));
+    LVSA_CUDA_TRY(cudaMemcpyAsync(oh, s_o, bytes, cudaMemcpyDeviceToHost, stream));
+    if (lseh != nullptr) LVSA_CUDA_TRY(cudaMemcpyAsync(lseh, s_lse, lbytes, cudaMemcpyDeviceToHost, stream));
     LVSA_CUDA_TRY(cudaStreamSynchronize(stream));
     return LVSA_OK;
 }
 
+void lvsa_workspace_release(void) {
+    std::lock_guard<std::mutex> lock(g_ws_mutex);
+    if (g_ws.ptr != nullptr) cudaFree(g_ws.ptr);
+    g_ws.ptr = nullptr; g_ws.cap = 0; g_ws.device = -1;
+}
+
 void lvsa_index_destroy(lvsa_index_t *ix) {
     if (ix == nullptr) return;
-    cudaFree(ix->d_wlo); cudaFree(ix->d_whi); cudaFree(ix->d_abits); cudaFree(ix->d_meta);
-    cudaFree(ix->d_indptr); cudaFree(ix->d_indices); cudaFree(ix->d_flags);
-    cudaFree(ix->d_item_ptr); cudaFree(ix->d_item_tiles);
-    cudaFree(ix->s_q); cudaFree(ix->s_k); cudaFree(ix->s_v); cudaFree(ix->s_o); cudaFree(ix->s_lse);
+    if (ix->arena != nullptr) {
+        // stream-ordered free behind the work that used the index; if several streams used it,
+        // wait for the device first
+        if (ix->multi_stream) cudaDeviceSynchronize();
+        cudaFreeAsync(ix->arena, ix->last_stream);
+    }
     delete ix;
 }
 
 lvsa_status_t lvsa_index_info(const lvsa_index_t *ix, lvsa_index_info_t *info) {
     if (ix == nullptr || info == nullptr) { lvsa_set_error("NULL argument"); return LVSA_EINVAL; }
     memset(info, 0, sizeof(*info));
+    lvsa_status_t fst = lvsa_index_fetch_meta(ix);
+    if (fst != LVSA_OK) return fst;
     const lvsa_params_t &p = ix->p;
     info->T = p.T; info->P = p.P; info->H = p.H; info->d = p.d; info->B = p.B;
     info->window = p.window; info->anchors = p.anchors; info->step = p.step; info->layer = p.layer;
@@ -166,6 +192,8 @@ lvsa_status_t lvsa_index_copy_host(const lvsa_index_t *ix, int32_t *indptr, int3
                                    uint8_t *flags, int32_t *w_lo, int32_t *w_hi, uint32_t *a_bits) {
     if (ix == nullptr) { lvsa_set_error("NULL index"); return LVSA_EINVAL; }
     const int T = ix->p.T;
+    lvsa_status_t fst = lvsa_index_fetch_meta(ix);
+    if (fst != LVSA_OK) return fst;
     if (indptr) LVSA_CUDA_TRY(cudaMemcpy(indptr, ix->d_indptr, sizeof(int32_t) * ((size_t)ix->nq + 1), cudaMemcpyDeviceToHost));
     if (indices && ix->nnz) LVSA_CUDA_TRY(cudaMemcpy(indices, ix->d_indices, sizeof(int32_t) * (size_t)ix->nnz, cudaMemcpyDeviceToHost));
     if (flags && ix->nnz) LVSA_CUDA_TRY(cudaMemcpy(flags, ix->d_flags, (size_t)ix->nnz, cudaMemcpyDeviceToHost));

@@ -95,6 +95,7 @@ __global__ void lvsa_tiles_kernel(long long N, int P, int Bq, int Bk, int nk, in
     const long long r1 = min(r0 + Bq, N) - 1;
     const int f0 = (int)(r0 / P), f1 = (int)(r1 / P);
     int running = 0, n_part = 0;
+    if (FILL && meta[7]) return;   // allocation bound exceeded (reported by the host)
     const int base = FILL ? indptr[i] : 0;
     for (int j0 = 0; j0 < nk; j0 += blockDim.x) {
         const int j = j0 + tid;
@@ -135,8 +136,10 @@ __global__ void lvsa_tiles_kernel(long long N, int P, int Bq, int Bk, int nk, in
 }
 
 // Single-block exclusive scan: out[0..n] from counts[0..n-1]; total also to *total_out.
+// If the total exceeds `cap` (the host's allocation bound) meta[7] is raised and the fill passes
+// write nothing; the host reports it at the next lvsa_index_info / copy_host.
 __global__ void lvsa_scan_kernel(const int32_t *__restrict__ counts, int n, int32_t *__restrict__ out,
-                                 int32_t *__restrict__ total_out) {
+                                 int32_t *__restrict__ total_out, long long cap, int32_t *__restrict__ overflow) {
     __shared__ int warp_tot[32];
     __shared__ int carry_s;
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5, nwarps = blockDim.x >> 5;
@@ -160,7 +163,7 @@ __global__ void lvsa_scan_kernel(const int32_t *__restrict__ counts, int n, int3
         if (tid == 0) carry_s = carry + tot;
         __syncthreads();
     }
-    if (tid == 0) { out[n] = carry_s; *total_out = carry_s; }
+    if (tid == 0) { out[n] = carry_s; *total_out = carry_s; if (carry_s > cap) *overflow = 1; }
 }
 
 // One thread per work item: union of the kv-tile lists of `group` (1 or 2) adjacent q tiles,
@@ -171,9 +174,9 @@ __global__ void lvsa_items_kernel(int nq, int group, long long n_items,
                                   const int32_t *__restrict__ indices,
                                   const uint8_t *__restrict__ flags,
                                   const int32_t *__restrict__ item_ptr, int32_t *__restrict__ counts,
-                                  int32_t *__restrict__ item_tiles) {
+                                  int32_t *__restrict__ item_tiles, const int32_t *__restrict__ overflow) {
     const long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (g >= n_items) return;
+    if (g >= n_items || *overflow) return;
     const int i0 = (int)(g * group), i1 = i0 + 1;
     int a = indptr[i0], ae = indptr[i0 + 1];
     int b = 0, be = 0;
@@ -194,59 +197,112 @@ __global__ void lvsa_items_kernel(int nq, int group, long long n_items,
 
 }  // namespace
 
+
+// Host side.  The whole build is enqueued on `stream` with no host synchronisation: buffers come
+// from one stream-ordered arena sized by an upper bound on the number of kept tiles, and the
+// counts the host wants to report (nnz, ...) are fetched lazily by lvsa_index_fetch_meta.
+//
+// Bound (allocation only; the pattern itself is computed on the device): a q tile touches at
+// most fq = floor((Bq-1)/P) + 2 frames, each attends to |A| <= min(T, m + 2W + 1) frames
+// (PAPER.md:66 closed form, m = |G| <= ceil(T / T_per)), and a frame overlaps at most
+// kf = floor((P-1)/Bk) + 2 kv tiles.
+static size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
+
 lvsa_status_t lvsa_index_build_device(lvsa_index *ix, cudaStream_t stream) {
     const lvsa_params_t &p = ix->p;
     const int T = p.T, words = ix->words;
-    LVSA_CUDA_TRY(cudaMalloc(&ix->d_wlo, sizeof(int32_t) * T));
-    LVSA_CUDA_TRY(cudaMalloc(&ix->d_whi, sizeof(int32_t) * T));
-    LVSA_CUDA_TRY(cudaMalloc(&ix->d_abits, sizeof(uint32_t) * (size_t)T * words));
-    LVSA_CUDA_TRY(cudaMalloc(&ix->d_meta, sizeof(int32_t) * 8));
-    LVSA_CUDA_TRY(cudaMemsetAsync(ix->d_meta, 0, sizeof(int32_t) * 8, stream));
-    LVSA_CUDA_TRY(cudaMalloc(&ix->d_indptr, sizeof(int32_t) * ((size_t)ix->nq + 1)));
-    int32_t *d_counts = nullptr;
-    LVSA_CUDA_TRY(cudaMalloc(&d_counts, sizeof(int32_t) * ((size_t)ix->nq + 1)));
-
     const int W = p.window > T ? T : p.window;  // W >= T already spans [0, T-1]; avoids 2W overflow
+
+    long long m_bound = T;
+    if (p.anchors >= 0 && p.anchors < T) {
+        if (p.anchors == 0) m_bound = 0;
+        else { const long long T_per = (T + p.anchors - 1) / p.anchors; m_bound = (T + T_per - 1) / T_per; }
+    }
+    long long a_bound = m_bound + 2ll * W + 1; if (a_bound > T) a_bound = T;
+    const long long fq = (p.tile_q - 1) / p.P + 2, kf = (p.P - 1) / p.tile_k + 2;
+    long long per_q = fq * a_bound * kf; if (per_q > ix->nk) per_q = ix->nk;
+    ix->n_items = (ix->nq + ix->group - 1) / ix->group;
+    long long per_item = per_q * ix->group; if (per_item > ix->nk) per_item = ix->nk;
+    ix->cap_nnz = per_q * ix->nq;
+    ix->cap_item_tiles = per_item * ix->n_items;
+    if (ix->cap_nnz >= (1ll << 31) || ix->cap_item_tiles >= (1ll << 31)) {
+        lvsa_set_error("index too large for int32 offsets");
+        return LVSA_EUNSUPPORTED;
+    }
+
+    const size_t n_counts = (size_t)(ix->nq > ix->n_items ? ix->nq : ix->n_items) + 1;
+    size_t off = 0;
+    auto take = [&](size_t bytes) { const size_t o = off; off += align_up(bytes); return o; };
+    const size_t o_wlo = take(sizeof(int32_t) * T), o_whi = take(sizeof(int32_t) * T);
+    const size_t o_abits = take(sizeof(uint32_t) * (size_t)T * words), o_meta = take(sizeof(int32_t) * 8);
+    const size_t o_indptr = take(sizeof(int32_t) * ((size_t)ix->nq + 1));
+    const size_t o_counts = take(sizeof(int32_t) * n_counts);
+    const size_t o_indices = take(sizeof(int32_t) * (size_t)(ix->cap_nnz + 1));
+    const size_t o_flags = take((size_t)(ix->cap_nnz + 1));
+    const size_t o_item_ptr = take(sizeof(int32_t) * ((size_t)ix->n_items + 1));
+    const size_t o_item_tiles = take(sizeof(int32_t) * (size_t)(ix->cap_item_tiles + 1));
+
+    static bool pool_ready[64] = {};
+    if (ix->device >= 0 && ix->device < 64 && !pool_ready[ix->device]) {
+        cudaMemPool_t pool;
+        LVSA_CUDA_TRY(cudaDeviceGetDefaultMemPool(&pool, ix->device));
+        unsigned long long keep = ~0ull;   // keep freed arenas cached: rebuilds then allocate in microseconds
+        LVSA_CUDA_TRY(cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep));
+        pool_ready[ix->device] = true;
+    }
+    LVSA_CUDA_TRY(cudaMallocAsync(&ix->arena, off, stream));
+    ix->arena_bytes = off;
+    ix->build_stream = stream;
+    ix->last_stream = stream;
+    uint8_t *a = static_cast<uint8_t *>(ix->arena);
+    ix->d_wlo = (int32_t *)(a + o_wlo); ix->d_whi = (int32_t *)(a + o_whi);
+    ix->d_abits = (uint32_t *)(a + o_abits); ix->d_meta = (int32_t *)(a + o_meta);
+    ix->d_indptr = (int32_t *)(a + o_indptr);
+    int32_t *d_counts = (int32_t *)(a + o_counts);
+    ix->d_indices = (int32_t *)(a + o_indices); ix->d_flags = a + o_flags;
+    ix->d_item_ptr = (int32_t *)(a + o_item_ptr); ix->d_item_tiles = (int32_t *)(a + o_item_tiles);
+
+    LVSA_CUDA_TRY(cudaMemsetAsync(ix->d_meta, 0, sizeof(int32_t) * 8, stream));
     lvsa_frames_kernel<<<1, 256, sizeof(uint32_t) * words, stream>>>(
         T, W, p.anchors, p.step, p.tie_break == LVSA_TIE_HI, words, ix->d_wlo, ix->d_whi,
         ix->d_abits, ix->d_meta);
     lvsa_tiles_kernel<false><<<ix->nq, 256, 0, stream>>>(
         (long long)ix->N, p.P, p.tile_q, p.tile_k, ix->nk, words, ix->d_abits, nullptr, d_counts,
         nullptr, nullptr, ix->d_meta);
-    lvsa_scan_kernel<<<1, 1024, 0, stream>>>(d_counts, ix->nq, ix->d_indptr, ix->d_meta + 0);
-    int32_t meta[8];
-    LVSA_CUDA_TRY(cudaMemcpyAsync(meta, ix->d_meta, sizeof(meta), cudaMemcpyDeviceToHost, stream));
-    LVSA_CUDA_TRY(cudaStreamSynchronize(stream));  // the one sync: learn nnz
-    LVSA_CUDA_TRY(cudaGetLastError());
-    ix->nnz = meta[0];
-    ix->T_per = meta[4]; ix->phase = meta[5]; ix->n_global = meta[6];
-    const size_t nnz_alloc = ix->nnz > 0 ? (size_t)ix->nnz : 1;
-    LVSA_CUDA_TRY(cudaMalloc(&ix->d_indices, sizeof(int32_t) * nnz_alloc));
-    LVSA_CUDA_TRY(cudaMalloc(&ix->d_flags, nnz_alloc));
+    lvsa_scan_kernel<<<1, 1024, 0, stream>>>(d_counts, ix->nq, ix->d_indptr, ix->d_meta + 0,
+                                             (long long)ix->cap_nnz, ix->d_meta + 7);
     lvsa_tiles_kernel<true><<<ix->nq, 256, 0, stream>>>(
         (long long)ix->N, p.P, p.tile_q, p.tile_k, ix->nk, words, ix->d_abits, ix->d_indptr, nullptr,
         ix->d_indices, ix->d_flags, ix->d_meta);
 
     // work items for the attention kernel
-    ix->n_items = (ix->nq + ix->group - 1) / ix->group;
-    LVSA_CUDA_TRY(cudaMalloc(&ix->d_item_ptr, sizeof(int32_t) * ((size_t)ix->n_items + 1)));
     const int ib = 128, ig = (int)((ix->n_items + ib - 1) / ib);
     lvsa_items_kernel<false><<<ig, ib, 0, stream>>>(ix->nq, ix->group, (long long)ix->n_items,
                                                      ix->d_indptr, ix->d_indices, ix->d_flags,
-                                                     nullptr, d_counts, nullptr);
+                                                     nullptr, d_counts, nullptr, ix->d_meta + 7);
     lvsa_scan_kernel<<<1, 1024, 0, stream>>>(d_counts, (int)ix->n_items, ix->d_item_ptr,
-                                             ix->d_meta + 2);
-    LVSA_CUDA_TRY(cudaMemcpyAsync(meta, ix->d_meta, sizeof(meta), cudaMemcpyDeviceToHost, stream));
-    LVSA_CUDA_TRY(cudaStreamSynchronize(stream));
-    ix->n_partial = meta[1];
-    ix->n_item_tiles = meta[2];
-    LVSA_CUDA_TRY(cudaMalloc(&ix->d_item_tiles,
-                             sizeof(int32_t) * (ix->n_item_tiles > 0 ? (size_t)ix->n_item_tiles : 1)));
+                                             ix->d_meta + 2, (long long)ix->cap_item_tiles, ix->d_meta + 7);
     lvsa_items_kernel<true><<<ig, ib, 0, stream>>>(ix->nq, ix->group, (long long)ix->n_items,
                                                     ix->d_indptr, ix->d_indices, ix->d_flags,
-                                                    ix->d_item_ptr, nullptr, ix->d_item_tiles);
-    LVSA_CUDA_TRY(cudaStreamSynchronize(stream));
+                                                    ix->d_item_ptr, nullptr, ix->d_item_tiles, ix->d_meta + 7);
     LVSA_CUDA_TRY(cudaGetLastError());
-    cudaFree(d_counts);
+    ix->meta_fetched = false;
+    return LVSA_OK;
+}
+
+// Reads the device-side counters (nnz, PARTIAL count, item entries, T_per, phase, |G|) once;
+// synchronises the build stream.  Called by lvsa_index_info / lvsa_index_copy_host.
+lvsa_status_t lvsa_index_fetch_meta(const lvsa_index *ix) {
+    if (ix->meta_fetched) return LVSA_OK;
+    int32_t meta[8];
+    LVSA_CUDA_TRY(cudaMemcpyAsync(meta, ix->d_meta, sizeof(meta), cudaMemcpyDeviceToHost, ix->build_stream));
+    LVSA_CUDA_TRY(cudaStreamSynchronize(ix->build_stream));
+    if (meta[7] != 0) {
+        lvsa_set_error("internal: kept-tile count exceeds the allocation bound");
+        return LVSA_ECUDA;
+    }
+    ix->nnz = meta[0]; ix->n_partial = meta[1]; ix->n_item_tiles = meta[2];
+    ix->T_per = meta[4]; ix->phase = meta[5]; ix->n_global = meta[6];
+    ix->meta_fetched = true;
     return LVSA_OK;
 }

@@ -20,10 +20,20 @@ struct lvsa_index {
     lvsa_params_t p;  // with defaults resolved
     int64_t N = 0;
     int32_t nq = 0, nk = 0, words = 0;
-    int32_t T_per = 0, phase = 0, n_global = 0;
-    int64_t nnz = 0, n_partial = 0;
+    // counters computed on the device; fetched lazily (lvsa_index_fetch_meta) so that the build
+    // itself never synchronises
+    mutable int32_t T_per = 0, phase = 0, n_global = 0;
+    mutable int64_t nnz = 0, n_partial = 0;
+    mutable bool meta_fetched = false;
     int device = 0;
-    // device buffers (owned)
+    // one stream-ordered arena holds every device buffer below
+    void *arena = nullptr;
+    size_t arena_bytes = 0;
+    int64_t cap_nnz = 0, cap_item_tiles = 0;   // allocation bounds (entries)
+    cudaStream_t build_stream = nullptr;
+    mutable cudaStream_t last_stream = nullptr;   // last stream that used the index
+    mutable bool multi_stream = false;            // used on more than one stream: free synchronously
+    // device buffers (views into the arena)
     int32_t *d_wlo = nullptr, *d_whi = nullptr;
     uint32_t *d_abits = nullptr;   // [T][words]
     int32_t *d_meta = nullptr;     // small scratch: {nnz, n_partial, n_item_tiles, n_global}
@@ -32,12 +42,10 @@ struct lvsa_index {
     uint8_t *d_flags = nullptr;    // [nnz]
     // attention work items: groups of LVSA_GROUP adjacent q tiles that share kv-tile loads
     int32_t group = 2;
-    int64_t n_items = 0, n_item_tiles = 0;
+    int64_t n_items = 0;
+    mutable int64_t n_item_tiles = 0;
     int32_t *d_item_ptr = nullptr;    // [n_items+1]
     int32_t *d_item_tiles = nullptr;  // [n_item_tiles], encoding above
-    // scratch for lvsa_attn_fwd_host (allocated on first use)
-    void *s_q = nullptr, *s_k = nullptr, *s_v = nullptr, *s_o = nullptr;
-    float *s_lse = nullptr;
 };
 
 void lvsa_set_error(const std::string &msg);
@@ -51,6 +59,7 @@ lvsa_status_t lvsa_cuda_fail(cudaError_t e, const char *what);
 
 // lvsa_index.cu
 lvsa_status_t lvsa_index_build_device(lvsa_index *ix, cudaStream_t stream);
+lvsa_status_t lvsa_index_fetch_meta(const lvsa_index *ix);
 
 // lvsa_attn_simt.cu
 lvsa_status_t lvsa_attn_simt_launch(const lvsa_index *ix, const void *q, const void *k,

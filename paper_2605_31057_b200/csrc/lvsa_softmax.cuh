@@ -104,6 +104,9 @@ __device__ __forceinline__ void exp_chunk32(const float (&s)[NC], int c0, uint64
     for (int x = 0; x < 16; ++x) {
         const uint64_t xv = fma2(pack2(s[c0 + 2 * x], s[c0 + 2 * x + 1]), scale2, negm2);
         float p0, p1;
+#ifdef LVSA_DIAG_NOEXP   // timing diagnostic only (wrong results): no exponential at all
+        unpack2(xv, p0, p1);
+#else
         if (pair_uses_poly<POLY>(x)) {
             poly_exp2_pair(xv, p0, p1);
         } else {
@@ -112,6 +115,7 @@ __device__ __forceinline__ void exp_chunk32(const float (&s)[NC], int c0, uint64
             p0 = fast_exp2(a);
             p1 = fast_exp2(b);
         }
+#endif
         lsum = add2(lsum, pack2(p0, p1));
         pk[x] = pack_bf16x2(p0, p1);
     }

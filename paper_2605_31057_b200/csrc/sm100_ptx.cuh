@@ -59,7 +59,7 @@ __device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
 }
 // Bounded wait: a protocol bug traps (launch fails with an error) instead of hanging the GPU.
 #ifndef LVSA_MBAR_SPIN_LIMIT
-#define LVSA_MBAR_SPIN_LIMIT (1u << 22)
+#define LVSA_MBAR_SPIN_LIMIT (1u << 17)
 #endif
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
     if (mbar_try_wait(bar, parity)) return;
