@@ -59,6 +59,11 @@ typedef struct lvsa_params {
                            (SIMT kernel only)                                                   */
     int32_t kernel;     /* LVSA_KERNEL_AUTO: tcgen05 for bf16, SIMT for fp32                    */
     float softmax_scale;/* default 1/sqrt(d) (Eq. 1)                                            */
+    int32_t initial_anchors; /* k0 >= 0 dedicated initial anchors: frames 0..k0-1 join G^s at every
+                           step (reading R22).  0 = the paper's pattern */
+    int32_t n_text;     /* >= 0 extra tokens after the T*P video tokens (HunyuanVideo's text tokens
+                           inside self-attention).  Every query attends to them and they
+                           attend to every token (reading R23).  N = T*P + n_text.          */
 } lvsa_params_t;
 
 typedef struct lvsa_index_info {
@@ -69,9 +74,11 @@ typedef struct lvsa_index_info {
     int32_t T_per;           /* 0 when there are no anchors                                     */
     int32_t phase;           /* s mod T_per                                                     */
     int32_t n_global;        /* |G^s|                                                           */
-    int32_t words;           /* uint32 words per A(t) bitset = ceil(T/32)                       */
+    int32_t words;           /* uint32 words per A(t) bitset = ceil(T'/32), T' = T + (n_text>0) */
     int32_t dtype, kernel;
-    int64_t N;               /* T*P                                                             */
+    int32_t n_text;          /* text tokens after the video tokens (R23)                        */
+    int32_t initial_anchors; /* dedicated initial anchors k0 (R22)                              */
+    int64_t N;               /* T*P + n_text                                                    */
     int64_t nnz;             /* kept (q tile, kv tile) pairs                                    */
     int64_t n_partial;       /* of which PARTIAL                                                */
     int64_t n_items;         /* work items of the attention kernel (q-tile groups)              */
@@ -129,6 +136,27 @@ lvsa_status_t lvsa_attn_fwd(const void *q, const void *k, const void *v,
 lvsa_status_t lvsa_attn_fwd_host(const void *q_host, const void *k_host, const void *v_host,
                                  lvsa_index_t *index, void *out_host, float *lse_host,
                                  void *stream);
+
+/*
+ * Whole-schedule driver.  The pattern of step s depends on s only
+ * through s mod T_per (Eq. 3), so a schedule of S denoising steps x L layers uses at
+ * most T_per distinct indices.  Where the paper recomputes the metadata on the CPU at every step
+ * (PAPER.md:104-110), lvsa_schedule_create builds all T_per indices once, on `stream`, without
+ * synchronising; lvsa_schedule_attn_fwd then only launches the attention kernel, which makes a
+ * whole S x L replay capturable in a CUDA graph (no allocation, no synchronisation, no index
+ * build inside the captured region).  `params->step` is ignored.
+ */
+typedef struct lvsa_schedule lvsa_schedule_t;
+lvsa_status_t lvsa_schedule_create(const lvsa_params_t *params, void *stream, lvsa_schedule_t **out);
+/* number of distinct phases = T_per (1 when there are no rotating anchors); 0 on NULL */
+int lvsa_schedule_num_phases(const lvsa_schedule_t *sched);
+/* the index of denoising step `step` >= 0 (borrowed: owned by the schedule); NULL on error */
+const lvsa_index_t *lvsa_schedule_index(const lvsa_schedule_t *sched, int step);
+/* lvsa_attn_fwd with the index of `step`; same argument rules; enqueue only */
+lvsa_status_t lvsa_schedule_attn_fwd(const lvsa_schedule_t *sched, int step, const void *q,
+                                     const void *k, const void *v, void *out, float *lse,
+                                     void *stream);
+void lvsa_schedule_destroy(lvsa_schedule_t *sched);
 
 /* Frees the device workspace of lvsa_attn_fwd_host (synchronises the device).  Safe to call
  * at any time when no lvsa_attn_fwd_host call is in flight; the next host call re-allocates. */

@@ -87,10 +87,15 @@ void lvsa_oracle_window(int T, int W, const uint8_t *inG, int nG, int tie_hi, in
 }
 
 /* ---- O5: A(t) = G^s u [w_lo(t), w_hi(t)] as a T x T 0/1 matrix, row t = query frame ------ */
-/* a == LVSA_ORACLE_ALL_TILES: A(t) = all frames (Def. 1). */
-void lvsa_oracle_pattern(int T, int W, int a, int s, int tie_hi,
-                         uint8_t *A, int32_t *w_lo, int32_t *w_hi, uint8_t *inG,
-                         int32_t *iters, int32_t *meta)
+/* a == LVSA_ORACLE_ALL_TILES: A(t) = all frames (Def. 1).
+ * k0 = number of dedicated initial anchors ("frame 0 is always a global anchor",
+ * :58 "an extension including more dedicated initial anchors is a straightforward
+ * generalization"; reading R22): G' = G^s u {0, ..., min(k0,T)-1}.  Frames of G' are
+ * the "global" frames of Algorithm 1 (its target and its non-global count use |G'|); T_per is
+ * still derived from a alone.  k0 = 0 is the paper's pattern.  meta[2] = |G'| (counted). */
+void lvsa_oracle_pattern_ex(int T, int W, int a, int s, int tie_hi, int k0,
+                            uint8_t *A, int32_t *w_lo, int32_t *w_hi, uint8_t *inG,
+                            int32_t *iters, int32_t *meta)
 {
     if (a == LVSA_ORACLE_ALL_TILES) {
         memset(A, 1, (size_t)T * T);
@@ -100,11 +105,31 @@ void lvsa_oracle_pattern(int T, int W, int a, int s, int tie_hi,
         return;
     }
     lvsa_oracle_anchor_set(T, a, s, inG, meta);
+    for (int f = 0; f < k0 && f < T; ++f) inG[f] = 1;
+    int cnt = 0;
+    for (int t = 0; t < T; ++t) cnt += inG[t];
+    meta[2] = cnt;
     for (int t = 0; t < T; ++t) {
         lvsa_oracle_window(T, W, inG, meta[2], tie_hi, t, &w_lo[t], &w_hi[t], &iters[t]);
         for (int x = 0; x < T; ++x)
             A[(size_t)t * T + x] = (uint8_t)(inG[x] || (x >= w_lo[t] && x <= w_hi[t]));
     }
+}
+
+void lvsa_oracle_pattern(int T, int W, int a, int s, int tie_hi,
+                         uint8_t *A, int32_t *w_lo, int32_t *w_hi, uint8_t *inG,
+                         int32_t *iters, int32_t *meta)
+{
+    lvsa_oracle_pattern_ex(T, W, a, s, tie_hi, 0, A, w_lo, w_hi, inG, iters, meta);
+}
+
+/* ---- token -> frame (reading R12), with the text extension (reading R23) ------ */
+/* Video token n = t*P + p belongs to frame t.  When n_text > 0 the n_text tokens after the T*P
+ * video tokens (HunyuanVideo's text tokens inside self-attention) form one
+ * pseudo-frame with index T; A then has T+1 rows/columns, row T and column T all ones. */
+static inline int64_t frame_of(int64_t n, int T, int P)
+{
+    return n < (int64_t)T * P ? n / P : T;
 }
 
 /* ---- O7: tile index straight from the definition -------------------------------------- */
@@ -116,21 +141,24 @@ void lvsa_oracle_pattern(int T, int W, int a, int s, int tie_hi,
  * "exists a pair of frames present in the two tiles"; the frame lists are found by walking
  * every token of the tile.  No interval arithmetic.
  * indices == NULL: count only.  Returns nnz, or -1 if cap is too small. */
-int64_t lvsa_oracle_tile_index(int T, int P, int Bq, int Bk, const uint8_t *A,
+int64_t lvsa_oracle_tile_index(int T, int P, int n_text, int Bq, int Bk, const uint8_t *A,
                                int32_t *indptr, int32_t *indices, uint8_t *flags, int64_t cap)
 {
-    const int64_t N = (int64_t)T * P;
+    /* A is Tf x Tf, Tf = T + (n_text > 0) */
+    const int64_t N = (int64_t)T * P + n_text;
+    const int Tv = T;
+    T = T + (n_text > 0 ? 1 : 0);
     const int64_t nq = (N + Bq - 1) / Bq, nk = (N + Bk - 1) / Bk;
     uint8_t *fq = (uint8_t *)malloc((size_t)T), *fk = (uint8_t *)malloc((size_t)T);
     /* frames present among the valid columns of every kv tile, nk x T */
     uint8_t *kfr = (uint8_t *)calloc((size_t)nk * T, 1);
     for (int64_t j = 0; j < nk; ++j)
-        for (int64_t c = j * Bk; c < (j + 1) * Bk && c < N; ++c) kfr[j * T + c / P] = 1;
+        for (int64_t c = j * Bk; c < (j + 1) * Bk && c < N; ++c) kfr[j * T + frame_of(c, Tv, P)] = 1;
     int64_t nnz = 0;
     for (int64_t i = 0; i < nq; ++i) {
         if (indptr) indptr[i] = (int32_t)nnz;
         memset(fq, 0, (size_t)T);
-        for (int64_t r = i * Bq; r < (i + 1) * Bq && r < N; ++r) fq[r / P] = 1;
+        for (int64_t r = i * Bq; r < (i + 1) * Bq && r < N; ++r) fq[frame_of(r, Tv, P)] = 1;
         for (int64_t j = 0; j < nk; ++j) {
             memcpy(fk, kfr + j * T, (size_t)T);
             int any_allowed = 0, any_disallowed = ((j + 1) * Bk > N);
@@ -172,11 +200,13 @@ static inline double ld_elem(const void *base, int is_bf16, int64_t e)
  * The key set is taken from the token predicate M directly (not from the tile list).
  * scale <= 0 means 1/sqrt(d) (Eq. 1). */
 void lvsa_oracle_attn_rows(const void *q, const void *k, const void *v, int is_bf16,
-                           int T, int P, int H, int d, const uint8_t *A,
+                           int T, int P, int n_text, int H, int d, const uint8_t *A,
                            const int64_t *rows, int64_t nrows, double scale,
                            double *out, double *lse, int nthreads)
 {
-    const int64_t N = (int64_t)T * P;
+    /* A is Tf x Tf, Tf = T + (n_text > 0); q,k,v hold N = T*P + n_text tokens */
+    const int64_t N = (int64_t)T * P + n_text;
+    const int Tf = T + (n_text > 0 ? 1 : 0);
     if (scale <= 0.0) scale = 1.0 / sqrt((double)d);
 #ifdef _OPENMP
     if (nthreads > 0) omp_set_num_threads(nthreads);
@@ -190,12 +220,12 @@ void lvsa_oracle_attn_rows(const void *q, const void *k, const void *v, int is_b
         for (int64_t ri = 0; ri < nrows; ++ri) {
             for (int h = 0; h < H; ++h) {
                 const int64_t nqi = rows[ri];
-                const uint8_t *Arow = A + (size_t)(nqi / P) * T;
+                const uint8_t *Arow = A + (size_t)frame_of(nqi, T, P) * Tf;
                 for (int c = 0; c < d; ++c) qd[c] = ld_elem(q, is_bf16, (nqi * H + h) * d + c);
                 /* logits s_j = q.k_j / sqrt(d) over allowed keys, and their max */
                 double mx = -INFINITY;
                 for (int64_t n = 0; n < N; ++n) {
-                    if (!Arow[n / P]) continue;
+                    if (!Arow[frame_of(n, T, P)]) continue;
                     const int64_t e = (n * H + h) * d;
                     double dot = 0.0;
 #pragma omp simd reduction(+ : dot)
@@ -207,7 +237,7 @@ void lvsa_oracle_attn_rows(const void *q, const void *k, const void *v, int is_b
                 double L = 0.0;
                 for (int c = 0; c < d; ++c) acc[c] = 0.0;
                 for (int64_t n = 0; n < N; ++n) {
-                    if (!Arow[n / P]) continue;
+                    if (!Arow[frame_of(n, T, P)]) continue;
                     const double p = exp(sc[n] - mx);
                     const int64_t e = (n * H + h) * d;
                     L += p;
@@ -226,27 +256,28 @@ void lvsa_oracle_attn_rows(const void *q, const void *k, const void *v, int is_b
 /* Returns 1 iff { keys contributed through the tile list } == { n : M(nq, n) } for every row
  * in rows.  FULL tiles contribute every column of the tile without consulting M (that is what
  * a kernel does); PARTIAL tiles contribute columns c < N with M(nq, c). */
-int lvsa_oracle_csr_keyset_equal(int T, int P, int Bq, int Bk, const uint8_t *A,
+int lvsa_oracle_csr_keyset_equal(int T, int P, int n_text, int Bq, int Bk, const uint8_t *A,
                                  const int32_t *indptr, const int32_t *indices,
                                  const uint8_t *flags, const int64_t *rows, int64_t nrows)
 {
-    const int64_t N = (int64_t)T * P;
+    const int64_t N = (int64_t)T * P + n_text;
+    const int Tf = T + (n_text > 0 ? 1 : 0);
     uint8_t *via = (uint8_t *)malloc((size_t)N + (size_t)Bk);
     int ok = 1;
     for (int64_t ri = 0; ri < nrows && ok; ++ri) {
         const int64_t nqi = rows[ri];
-        const uint8_t *Arow = A + (size_t)(nqi / P) * T;
+        const uint8_t *Arow = A + (size_t)frame_of(nqi, T, P) * Tf;
         memset(via, 0, (size_t)N + (size_t)Bk);
         const int64_t i = nqi / Bq;
         for (int32_t e = indptr[i]; e < indptr[i + 1]; ++e) {
             const int64_t j = indices[e];
             for (int64_t c = j * Bk; c < (j + 1) * Bk; ++c) {
-                if (flags[e]) { if (c < N && Arow[c / P]) via[c] += 1; }
+                if (flags[e]) { if (c < N && Arow[frame_of(c, T, P)]) via[c] += 1; }
                 else          { via[c] += 1; }
             }
         }
         for (int64_t n = 0; n < N + Bk; ++n) {
-            const int want = (n < N) ? Arow[n / P] : 0;
+            const int want = (n < N) ? Arow[frame_of(n, T, P)] : 0;
             if (via[n] != want) { ok = 0; break; }
         }
     }

@@ -92,30 +92,45 @@ class Pattern:
         return out
 
 
-def pattern(T: int, W: int, a: int, s: int, tie_hi: int = 0) -> Pattern:
+def pattern(T: int, W: int, a: int, s: int, tie_hi: int = 0, initial_anchors: int = 0) -> Pattern:
+    """Def. 2 with Eq. 3 and Algorithm 1; initial_anchors = k0 dedicated first frames added to
+    G^s (reading R22; 0 = the paper's pattern)."""
     A = np.zeros((T, T), np.uint8)
     lo = np.zeros(T, np.int32)
     hi = np.zeros(T, np.int32)
     inG = np.zeros(T, np.uint8)
     it = np.zeros(T, np.int32)
     meta = np.zeros(3, np.int32)
-    lib().lvsa_oracle_pattern(C.c_int(T), C.c_int(W), C.c_int(a), C.c_int(s), C.c_int(tie_hi),
-                              _p(A), _p(lo), _p(hi), _p(inG), _p(it), _p(meta))
+    lib().lvsa_oracle_pattern_ex(C.c_int(T), C.c_int(W), C.c_int(a), C.c_int(s), C.c_int(tie_hi),
+                                 C.c_int(initial_anchors), _p(A), _p(lo), _p(hi), _p(inG), _p(it),
+                                 _p(meta))
     return Pattern(T, W, a, s, A, lo, hi, inG, it, int(meta[0]), int(meta[1]), int(meta[2]))
 
 
-def tile_index(T: int, P: int, Bq: int, Bk: int, A: np.ndarray):
-    """CSR (indptr, indices, flags) of kept kv tiles per q tile; flags 1 = PARTIAL."""
+def with_text(A: np.ndarray) -> np.ndarray:
+    """Frame-level pattern with the text pseudo-frame appended (reading R23 of
+    PAPER.md:132): every video frame attends to the text tokens, the text tokens attend to every
+    frame and to themselves.  [T, T] -> [T+1, T+1]."""
+    T = A.shape[0]
+    Af = np.ones((T + 1, T + 1), np.uint8)
+    Af[:T, :T] = A
+    return Af
+
+
+def tile_index(T: int, P: int, Bq: int, Bk: int, A: np.ndarray, n_text: int = 0):
+    """CSR (indptr, indices, flags) of kept kv tiles per q tile; flags 1 = PARTIAL.
+    n_text > 0: A is the [T+1, T+1] pattern of with_text and N = T*P + n_text."""
     A = np.ascontiguousarray(A, np.uint8)
-    N = T * P
+    assert A.shape == (T + (n_text > 0), T + (n_text > 0))
+    N = T * P + n_text
     nq = (N + Bq - 1) // Bq
     indptr = np.zeros(nq + 1, np.int32)
-    nnz = lib().lvsa_oracle_tile_index(C.c_int(T), C.c_int(P), C.c_int(Bq), C.c_int(Bk), _p(A),
-                                       _p(indptr), None, None, C.c_int64(0))
+    nnz = lib().lvsa_oracle_tile_index(C.c_int(T), C.c_int(P), C.c_int(n_text), C.c_int(Bq), C.c_int(Bk),
+                                       _p(A), _p(indptr), None, None, C.c_int64(0))
     indices = np.zeros(max(nnz, 1), np.int32)
     flags = np.zeros(max(nnz, 1), np.uint8)
-    got = lib().lvsa_oracle_tile_index(C.c_int(T), C.c_int(P), C.c_int(Bq), C.c_int(Bk), _p(A),
-                                       _p(indptr), _p(indices), _p(flags), C.c_int64(nnz))
+    got = lib().lvsa_oracle_tile_index(C.c_int(T), C.c_int(P), C.c_int(n_text), C.c_int(Bq), C.c_int(Bk),
+                                       _p(A), _p(indptr), _p(indices), _p(flags), C.c_int64(nnz))
     assert got == nnz
     return indptr, indices[:nnz], flags[:nnz]
 
@@ -131,7 +146,7 @@ def _as_input(x) -> tuple[np.ndarray, int]:
 
 
 def attn_rows(q, k, v, T: int, P: int, A: np.ndarray, rows, scale: float = 0.0,
-              nthreads: int = 0):
+              nthreads: int = 0, n_text: int = 0):
     """Eq. 2 for the query tokens in `rows`, every head.  q,k,v: [N, H, d].
     Returns (out [nrows,H,d] fp64, lse [nrows,H] fp64)."""
     q, b0 = _as_input(q)
@@ -139,26 +154,26 @@ def attn_rows(q, k, v, T: int, P: int, A: np.ndarray, rows, scale: float = 0.0,
     v, b2 = _as_input(v)
     assert b0 == b1 == b2 and q.shape == k.shape == v.shape and q.ndim == 3
     N, H, d = q.shape
-    assert N == T * P
+    assert N == T * P + n_text and A.shape[0] == T + (n_text > 0)
     A = np.ascontiguousarray(A, np.uint8)
     rows = np.ascontiguousarray(rows, np.int64)
     assert rows.size == 0 or (rows.min() >= 0 and rows.max() < N)
     out = np.zeros((rows.size, H, d), np.float64)
     lse = np.zeros((rows.size, H), np.float64)
     lib().lvsa_oracle_attn_rows(_p(q), _p(k), _p(v), C.c_int(b0), C.c_int(T), C.c_int(P),
-                                C.c_int(H), C.c_int(d), _p(A), _p(rows), C.c_int64(rows.size),
+                                C.c_int(n_text), C.c_int(H), C.c_int(d), _p(A), _p(rows), C.c_int64(rows.size),
                                 C.c_double(scale), _p(out), _p(lse), C.c_int(nthreads))
     return out, lse
 
 
-def csr_keyset_equal(T, P, Bq, Bk, A, indptr, indices, flags, rows) -> bool:
+def csr_keyset_equal(T, P, Bq, Bk, A, indptr, indices, flags, rows, n_text: int = 0) -> bool:
     A = np.ascontiguousarray(A, np.uint8)
     rows = np.ascontiguousarray(rows, np.int64)
     indptr = np.ascontiguousarray(indptr, np.int32)
     indices = np.ascontiguousarray(indices, np.int32)
     flags = np.ascontiguousarray(flags, np.uint8)
     return bool(lib().lvsa_oracle_csr_keyset_equal(
-        C.c_int(T), C.c_int(P), C.c_int(Bq), C.c_int(Bk), _p(A), _p(indptr), _p(indices),
+        C.c_int(T), C.c_int(P), C.c_int(n_text), C.c_int(Bq), C.c_int(Bk), _p(A), _p(indptr), _p(indices),
         _p(flags), _p(rows), C.c_int64(rows.size)))
 
 

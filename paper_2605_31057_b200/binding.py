@@ -33,19 +33,23 @@ class LvsaError(RuntimeError):
 class Params(C.Structure):
     _fields_ = [(n, C.c_int32) for n in
                 ("T", "P", "H", "d", "B", "window", "anchors", "step", "layer", "tile_q", "tile_k",
-                 "tie_break", "dtype", "kernel")] + [("softmax_scale", C.c_float)]
+                 "tie_break", "dtype", "kernel")] + [("softmax_scale", C.c_float),
+                                                     ("initial_anchors", C.c_int32),
+                                                     ("n_text", C.c_int32)]
 
 
 class IndexInfo(C.Structure):
     _fields_ = [(n, C.c_int32) for n in
                 ("T", "P", "H", "d", "B", "window", "anchors", "step", "layer", "tile_q", "tile_k",
-                 "nq", "nk", "T_per", "phase", "n_global", "words", "dtype", "kernel")] + \
+                 "nq", "nk", "T_per", "phase", "n_global", "words", "dtype", "kernel", "n_text",
+                 "initial_anchors")] + \
                [(n, C.c_int64) for n in ("N", "nnz", "n_partial", "n_items", "n_item_tiles")]
 
 
 EXPORTS = ("lvsa_build_block_index", "lvsa_build_block_index_ex", "lvsa_attn_fwd",
            "lvsa_attn_fwd_host", "lvsa_index_destroy", "lvsa_index_info", "lvsa_index_copy_host",
-           "lvsa_attn_fwd_launches", "lvsa_workspace_release", "lvsa_last_error", "lvsa_version")
+           "lvsa_attn_fwd_launches", "lvsa_workspace_release", "lvsa_schedule_create",
+           "lvsa_schedule_num_phases", "lvsa_schedule_index", "lvsa_schedule_attn_fwd", "lvsa_schedule_destroy", "lvsa_last_error", "lvsa_version")
 
 _lib = None
 
@@ -72,6 +76,18 @@ def lib() -> C.CDLL:
         L.lvsa_index_copy_host.argtypes = [C.c_void_p] * 7
         L.lvsa_attn_fwd_launches.restype = C.c_int
         L.lvsa_attn_fwd_launches.argtypes = [C.c_void_p]
+        L.lvsa_workspace_release.restype = None
+        L.lvsa_workspace_release.argtypes = []
+        L.lvsa_schedule_create.restype = C.c_int
+        L.lvsa_schedule_create.argtypes = [C.POINTER(Params), C.c_void_p, C.POINTER(C.c_void_p)]
+        L.lvsa_schedule_num_phases.restype = C.c_int
+        L.lvsa_schedule_num_phases.argtypes = [C.c_void_p]
+        L.lvsa_schedule_index.restype = C.c_void_p
+        L.lvsa_schedule_index.argtypes = [C.c_void_p, C.c_int]
+        L.lvsa_schedule_attn_fwd.restype = C.c_int
+        L.lvsa_schedule_attn_fwd.argtypes = [C.c_void_p, C.c_int] + [C.c_void_p] * 6
+        L.lvsa_schedule_destroy.restype = None
+        L.lvsa_schedule_destroy.argtypes = [C.c_void_p]
         L.lvsa_last_error.restype = C.c_char_p
         L.lvsa_version.restype = C.c_char_p
         _lib = L
@@ -102,10 +118,11 @@ class HostIndex:
 
 
 class BlockIndex:
-    """Owns one lvsa_index_t handle."""
+    """One lvsa_index_t handle: owned (destroyed with the object) unless borrowed from a schedule."""
 
-    def __init__(self, handle: int):
+    def __init__(self, handle: int, owned: bool = True):
         self._h = C.c_void_p(handle)
+        self._owned = owned
 
     @property
     def handle(self) -> C.c_void_p:
@@ -125,7 +142,7 @@ class BlockIndex:
         flags = np.zeros(i.nnz, np.uint8)
         w_lo = np.zeros(i.T, np.int32)
         w_hi = np.zeros(i.T, np.int32)
-        a_bits = np.zeros((i.T, i.words), np.uint32)
+        a_bits = np.zeros((i.T + (1 if i.n_text > 0 else 0), i.words), np.uint32)
         ptr = lambda a: a.ctypes.data_as(C.c_void_p)
         _check(lib().lvsa_index_copy_host(self.handle, ptr(indptr), ptr(indices), ptr(flags),
                                           ptr(w_lo), ptr(w_hi), ptr(a_bits)))
@@ -136,7 +153,8 @@ class BlockIndex:
 
     def destroy(self):
         if self._h:
-            lib().lvsa_index_destroy(self._h)
+            if self._owned:
+                lib().lvsa_index_destroy(self._h)
             self._h = C.c_void_p(None)
 
     def __del__(self):
@@ -193,4 +211,56 @@ def lvsa_attn_fwd_host(q, k, v, index: BlockIndex, out, lse=None, stream: int = 
             raise ValueError("lvsa_attn_fwd_host takes contiguous CPU tensors")
     _check(lib().lvsa_attn_fwd_host(hp(q), hp(k), hp(v), index.handle, hp(out), hp(lse),
                                     C.c_void_p(stream)))
+    return out
+
+
+def lvsa_workspace_release() -> None:
+    lib().lvsa_workspace_release()
+
+
+class Schedule:
+    """Owns one lvsa_schedule_t: the T_per distinct block indices of a denoising schedule."""
+
+    def __init__(self, handle: int):
+        self._h = C.c_void_p(handle)
+
+    @property
+    def handle(self) -> C.c_void_p:
+        if not self._h:
+            raise ValueError("schedule already destroyed")
+        return self._h
+
+    def num_phases(self) -> int:
+        return int(lib().lvsa_schedule_num_phases(self.handle))
+
+    def index(self, step: int) -> BlockIndex:
+        """Borrowed view of the index of `step` (do not destroy it)."""
+        h = lib().lvsa_schedule_index(self.handle, C.c_int(step))
+        if not h:
+            raise LvsaError(EINVAL, lvsa_last_error())
+        return BlockIndex(h, owned=False)
+
+    def destroy(self) -> None:
+        if self._h:
+            lib().lvsa_schedule_destroy(self._h)
+            self._h = C.c_void_p(None)
+
+
+def lvsa_schedule_create(stream: int = 0, **kw) -> Schedule:
+    p = Params()
+    for k, v in kw.items():
+        if not hasattr(p, k):
+            raise TypeError(f"unknown lvsa_params_t field {k!r}")
+        setattr(p, k, v)
+    out = C.c_void_p()
+    _check(lib().lvsa_schedule_create(C.byref(p), C.c_void_p(stream), C.byref(out)))
+    return Schedule(out.value)
+
+
+def lvsa_schedule_attn_fwd(sched: Schedule, step: int, q, k, v, out, lse=None, stream: int | None = None):
+    if stream is None:
+        import torch
+        stream = torch.cuda.current_stream().cuda_stream
+    _check(lib().lvsa_schedule_attn_fwd(sched.handle, C.c_int(step), _dev_ptr(q), _dev_ptr(k), _dev_ptr(v),
+                                        _dev_ptr(out), _dev_ptr(lse), C.c_void_p(stream)))
     return out

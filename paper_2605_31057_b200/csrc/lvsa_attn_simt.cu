@@ -29,7 +29,7 @@ lvsa_attn_simt_kernel(const T *__restrict__ q, const T *__restrict__ k, const T 
                       T *__restrict__ out, float *__restrict__ lse,
                       const int32_t *__restrict__ indptr, const int32_t *__restrict__ indices,
                       const uint8_t *__restrict__ flags, const uint32_t *__restrict__ a_bits,
-                      int words, long long N, int P, int H, float scale) {
+                      int words, long long N, int P, int Tf, int H, float scale) {
     constexpr int R = BT / SIMT_WARPS;  // rows per warp
     constexpr int CH = D / 32;          // output channels per lane
     constexpr int KS = D + 1;           // padded K row (lane c reads row c: conflict-free)
@@ -78,7 +78,7 @@ lvsa_attn_simt_kernel(const T *__restrict__ q, const T *__restrict__ k, const T 
             const int rl = wid + r * SIMT_WARPS;
             const long long nq = row0 + rl;
             if (nq >= N) continue;  // warp-uniform
-            const uint32_t *arow = a_bits + (size_t)(nq / P) * words;
+            const uint32_t *arow = a_bits + (size_t)min((int)(nq / P), Tf - 1) * words;   // text rows: frame Tf-1
             const float *qrow = Qs + rl * D;
             for (int cc = 0; cc < BT / 32; ++cc) {
                 const int cl = cc * 32 + lane;
@@ -90,7 +90,7 @@ lvsa_attn_simt_kernel(const T *__restrict__ q, const T *__restrict__ k, const T 
                 if (partial) {
                     const long long nk_ = col0 + cl;
                     bool ok = nk_ < N;
-                    if (ok) { const int f = (int)(nk_ / P); ok = (arow[f >> 5] >> (f & 31)) & 1u; }
+                    if (ok) { const int f = min((int)(nk_ / P), Tf - 1); ok = (arow[f >> 5] >> (f & 31)) & 1u; }
                     if (!ok) s = -INFINITY;
                 }
                 float cmax = s;
@@ -142,7 +142,7 @@ lvsa_status_t launch(const lvsa_index *ix, const void *q, const void *k, const v
     dim3 grid(ix->nq, ix->p.H, ix->p.B);
     kern<<<grid, SIMT_WARPS * 32, smem, stream>>>(
         (const T *)q, (const T *)k, (const T *)v, (T *)out, lse, ix->d_indptr, ix->d_indices,
-        ix->d_flags, ix->d_abits, ix->words, (long long)ix->N, ix->p.P, ix->p.H, scale);
+        ix->d_flags, ix->d_abits, ix->words, (long long)ix->N, ix->p.P, ix->Tf, ix->p.H, scale);
     LVSA_CUDA_TRY(cudaGetLastError());
     return LVSA_OK;
 }

@@ -163,11 +163,14 @@ lvsa_attn_sm100_v0_kernel(const __grid_constant__ CUtensorMap tmap_q,
                 for (int w = 0; w < BT / 32; ++w) cm[w] = 0u;
                 if (st_row == LVSA_ST_PARTIAL) {
                     const long long cend = min(col0 + BT, N);
-                    int g = (int)(col0 / P);
-                    for (long long fs = (long long)g * P; fs < cend; fs += P, ++g) {
+                    // frame g covers tokens [g P, (g+1) P); the last frame row (the text pseudo-frame when
+                    // n_text > 0, R23) runs to N
+                    int g = min((int)(col0 / P), T - 1);
+                    for (long long fs = (long long)g * P, fe; fs < cend; fs = fe, ++g) {
+                        fe = (g == T - 1) ? N : fs + P;
                         if ((arow[g >> 5] >> (g & 31)) & 1u) {
                             const int lo = (int)(max(fs, col0) - col0);
-                            const int hi = (int)(min(fs + P, cend) - col0);
+                            const int hi = (int)(min(fe, cend) - col0);
 #pragma unroll
                             for (int w = 0; w < BT / 32; ++w) cm[w] |= range_mask32(lo, hi, w);
                         }
@@ -322,7 +325,7 @@ lvsa_status_t launch_v0(const lvsa_index *ix, const void *q, const void *k, cons
     dim3 grid((unsigned)ix->n_items, ix->p.H, ix->p.B);
     kern<<<grid, C::NWG * 128, C::SMEM_BYTES, stream>>>(
         mq, mk, mv, (__nv_bfloat16 *)out, lse, ix->d_item_ptr, ix->d_item_tiles, ix->d_abits, ix->words,
-        (long long)ix->N, ix->p.P, ix->p.T, ix->p.H, scale_log2, g_dbg);
+        (long long)ix->N, ix->p.P, ix->Tf, ix->p.H, scale_log2, g_dbg);
     LVSA_CUDA_TRY(cudaGetLastError());
     return LVSA_OK;
 }
@@ -332,9 +335,17 @@ lvsa_status_t launch_v0(const lvsa_index *ix, const void *q, const void *k, cons
 extern "C" void lvsa_debug_set_dump(float *dev_ptr) { g_dbg = dev_ptr; }
 
 int lvsa_attn_sm100_supported(const lvsa_index *ix) {
-    cudaDeviceProp prop;
-    if (cudaGetDeviceProperties(&prop, ix->device) != cudaSuccess) return 0;
-    if (prop.major != 10) return 0;
+    // compute-capability major per device, queried once (cudaGetDeviceProperties costs milliseconds
+    // and this runs in every index build)
+    static int cc_major[64] = {};
+    const int dev = ix->device;
+    if (dev < 0 || dev >= 64) return 0;
+    if (cc_major[dev] == 0) {
+        int v = 0;
+        if (cudaDeviceGetAttribute(&v, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess) return 0;
+        cc_major[dev] = v;
+    }
+    if (cc_major[dev] != 10) return 0;
     return (ix->p.d == 128 && ix->p.tile_q == 128) || (ix->p.d == 64 && ix->p.tile_q == 64);
 }
 

@@ -140,10 +140,13 @@ lvsa_attn_sm100_ws_kernel(const __grid_constant__ CUtensorMap tmap_q,
                 if (st == LVSA_ST_PARTIAL) {
                     uint32_t cm[4] = {0u, 0u, 0u, 0u};
                     const long long cend = min(col0 + BT, N);
-                    int g = (int)(col0 / P);
-                    for (long long fs = (long long)g * P; fs < cend; fs += P, ++g) {
+                    // frame g covers tokens [g P, (g+1) P); the last frame row (the text pseudo-frame when
+                    // n_text > 0, R23) runs to N
+                    int g = min((int)(col0 / P), T - 1);
+                    for (long long fs = (long long)g * P, fe; fs < cend; fs = fe, ++g) {
+                        fe = (g == T - 1) ? N : fs + P;
                         if ((arow[g >> 5] >> (g & 31)) & 1u) {
-                            const int lo = (int)(max(fs, col0) - col0), hi = (int)(min(fs + P, cend) - col0);
+                            const int lo = (int)(max(fs, col0) - col0), hi = (int)(min(fe, cend) - col0);
 #pragma unroll
                             for (int x = 0; x < 4; ++x) cm[x] |= range_mask32(lo, hi, x);
                         }
@@ -400,6 +403,20 @@ lvsa_attn_sm100_ws_kernel(const __grid_constant__ CUtensorMap tmap_q,
 lvsa_status_t lvsa_make_tmap_bf16(CUtensorMap *m, const void *base, long long N, int H, int d, int B,
                                   int box_rows);
 
+// One-time setup (opt-in shared memory size, SM count), kept out of the launch path so that a
+// launch is nothing but tensor-map encoding and the launch itself (CUDA-graph capturable).
+static int g_n_sm = 0;
+lvsa_status_t lvsa_attn_sm100_ws_prepare(int device) {
+    if (g_n_sm != 0) return LVSA_OK;
+    using SM = Smem<5>;
+    LVSA_CUDA_TRY(cudaFuncSetAttribute(lvsa_attn_sm100_ws_kernel<5>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                       SM::BYTES));
+    int n = 0;
+    LVSA_CUDA_TRY(cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, device));
+    g_n_sm = n;
+    return LVSA_OK;
+}
+
 lvsa_status_t lvsa_attn_sm100_ws_launch(const lvsa_index *ix, const void *q, const void *k, const void *v,
                                         void *out, float *lse, cudaStream_t stream) {
     constexpr int NS = 5;
@@ -410,17 +427,14 @@ lvsa_status_t lvsa_attn_sm100_ws_launch(const lvsa_index *ix, const void *q, con
     if ((st = lvsa_make_tmap_bf16(&mk, k, ix->N, ix->p.H, D, ix->p.B, BT)) != LVSA_OK) return st;
     if ((st = lvsa_make_tmap_bf16(&mv, v, ix->N, ix->p.H, D, ix->p.B, BT)) != LVSA_OK) return st;
     auto kern = lvsa_attn_sm100_ws_kernel<NS>;
-    static int n_sm = 0;
-    if (n_sm == 0) {
-        LVSA_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, SM::BYTES));
-        LVSA_CUDA_TRY(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, ix->device));
-    }
+    if ((st = lvsa_attn_sm100_ws_prepare(ix->device)) != LVSA_OK) return st;
+    const int n_sm = g_n_sm;
     const long long n_work = (long long)ix->n_items * ix->p.H * ix->p.B;
     const int grid = (int)(n_work < n_sm ? n_work : n_sm);
     const float scale_log2 = ix->p.softmax_scale * 1.4426950408889634f;
     kern<<<grid, NTHREADS, SM::BYTES, stream>>>(
         mq, mk, mv, (__nv_bfloat16 *)out, lse, ix->d_item_ptr, ix->d_item_tiles, ix->d_abits, ix->words,
-        (long long)ix->N, ix->p.P, ix->p.T, ix->p.H, (int)ix->n_items, n_work, scale_log2);
+        (long long)ix->N, ix->p.P, ix->Tf, ix->p.H, (int)ix->n_items, n_work, scale_log2);
     LVSA_CUDA_TRY(cudaGetLastError());
     return LVSA_OK;
 }

@@ -28,6 +28,11 @@ static int use_tcgen05(const lvsa_index *ix) {
     return ix->p.dtype == LVSA_DTYPE_BF16;
 }
 
+lvsa_status_t lvsa_attn_prepare(const lvsa_index *ix) {
+    if (use_tcgen05(ix) && ix->p.d == 128) return lvsa_attn_sm100_ws_prepare(ix->device);
+    return LVSA_OK;   // the other kernels set their attributes at launch
+}
+
 extern "C" {
 
 const char *lvsa_last_error(void) { return g_last_error.c_str(); }
@@ -47,7 +52,9 @@ lvsa_status_t lvsa_build_block_index_ex(const lvsa_params_t *params, void *strea
     if (p.window < 0) { lvsa_set_error("window must be >= 0"); return LVSA_EINVAL; }
     if (p.anchors < LVSA_ANCHORS_ALL_TILES) { lvsa_set_error("anchors must be >= -1"); return LVSA_EINVAL; }
     if (p.step < 0 || p.layer < 0) { lvsa_set_error("step and layer must be >= 0"); return LVSA_EINVAL; }
-    if ((long long)p.T * p.P >= (1ll << 31)) { lvsa_set_error("T*P must be < 2^31"); return LVSA_EINVAL; }
+    if ((long long)p.T * p.P + (long long)(p.n_text > 0 ? p.n_text : 0) >= (1ll << 31)) { lvsa_set_error("T*P + n_text must be < 2^31"); return LVSA_EINVAL; }
+    if (p.initial_anchors < 0) { lvsa_set_error("initial_anchors must be >= 0"); return LVSA_EINVAL; }
+    if (p.n_text < 0) { lvsa_set_error("n_text must be >= 0"); return LVSA_EINVAL; }
     if (p.tie_break != LVSA_TIE_LO && p.tie_break != LVSA_TIE_HI) { lvsa_set_error("bad tie_break"); return LVSA_EINVAL; }
     if (p.dtype != LVSA_DTYPE_BF16 && p.dtype != LVSA_DTYPE_FP32) { lvsa_set_error("bad dtype"); return LVSA_EINVAL; }
     if (p.kernel < LVSA_KERNEL_AUTO || p.kernel > LVSA_KERNEL_TCGEN05) { lvsa_set_error("bad kernel"); return LVSA_EINVAL; }
@@ -68,10 +75,11 @@ lvsa_status_t lvsa_build_block_index_ex(const lvsa_params_t *params, void *strea
     lvsa_index *ix = new (std::nothrow) lvsa_index();
     if (ix == nullptr) { lvsa_set_error("out of host memory"); return LVSA_ENOMEM; }
     ix->p = p;
-    ix->N = (int64_t)p.T * p.P;
+    ix->N = (int64_t)p.T * p.P + p.n_text;
+    ix->Tf = p.T + (p.n_text > 0 ? 1 : 0);
     ix->nq = (int32_t)((ix->N + p.tile_q - 1) / p.tile_q);
     ix->nk = (int32_t)((ix->N + p.tile_k - 1) / p.tile_k);
-    ix->words = (p.T + 31) / 32;
+    ix->words = (ix->Tf + 31) / 32;
     ix->group = 2;
     if ((long long)ix->nq * ix->nk >= (1ll << 31)) {
         lvsa_index_destroy(ix);
@@ -181,7 +189,8 @@ lvsa_status_t lvsa_index_info(const lvsa_index_t *ix, lvsa_index_info_t *info) {
     info->window = p.window; info->anchors = p.anchors; info->step = p.step; info->layer = p.layer;
     info->tile_q = p.tile_q; info->tile_k = p.tile_k; info->nq = ix->nq; info->nk = ix->nk;
     info->T_per = ix->T_per; info->phase = ix->phase; info->n_global = ix->n_global;
-    info->words = ix->words; info->dtype = p.dtype;
+    info->words = ix->words; info->dtype = p.dtype; info->n_text = p.n_text;
+    info->initial_anchors = p.initial_anchors;
     info->kernel = use_tcgen05(ix) ? LVSA_KERNEL_TCGEN05 : LVSA_KERNEL_SIMT;
     info->N = ix->N; info->nnz = ix->nnz; info->n_partial = ix->n_partial;
     info->n_items = ix->n_items; info->n_item_tiles = ix->n_item_tiles;
@@ -199,8 +208,61 @@ lvsa_status_t lvsa_index_copy_host(const lvsa_index_t *ix, int32_t *indptr, int3
     if (flags && ix->nnz) LVSA_CUDA_TRY(cudaMemcpy(flags, ix->d_flags, (size_t)ix->nnz, cudaMemcpyDeviceToHost));
     if (w_lo) LVSA_CUDA_TRY(cudaMemcpy(w_lo, ix->d_wlo, sizeof(int32_t) * T, cudaMemcpyDeviceToHost));
     if (w_hi) LVSA_CUDA_TRY(cudaMemcpy(w_hi, ix->d_whi, sizeof(int32_t) * T, cudaMemcpyDeviceToHost));
-    if (a_bits) LVSA_CUDA_TRY(cudaMemcpy(a_bits, ix->d_abits, sizeof(uint32_t) * (size_t)T * ix->words, cudaMemcpyDeviceToHost));
+    if (a_bits) LVSA_CUDA_TRY(cudaMemcpy(a_bits, ix->d_abits, sizeof(uint32_t) * (size_t)ix->Tf * ix->words, cudaMemcpyDeviceToHost));
     return LVSA_OK;
+}
+
+// ---------------------------------------------------------------- whole-schedule driver (f1)
+struct lvsa_schedule {
+    int n_phases = 0;
+    lvsa_index **phase = nullptr;   // [n_phases], index of step r = phase r
+};
+
+lvsa_status_t lvsa_schedule_create(const lvsa_params_t *params, void *stream, lvsa_schedule_t **out) {
+    if (params == nullptr || out == nullptr) { lvsa_set_error("NULL argument"); return LVSA_EINVAL; }
+    *out = nullptr;
+    // a1: T_per = ceil(T / a); no rotation without anchors or on the all-tiles path
+    int n = 1;
+    if (params->T > 0 && params->anchors > 0) n = (params->T + params->anchors - 1) / params->anchors;
+    lvsa_schedule *sc = new (std::nothrow) lvsa_schedule();
+    if (sc == nullptr) { lvsa_set_error("out of host memory"); return LVSA_ENOMEM; }
+    sc->phase = new (std::nothrow) lvsa_index *[n]();
+    if (sc->phase == nullptr) { delete sc; lvsa_set_error("out of host memory"); return LVSA_ENOMEM; }
+    sc->n_phases = n;
+    for (int r = 0; r < n; ++r) {
+        lvsa_params_t p = *params;
+        p.step = r;
+        lvsa_status_t st = lvsa_build_block_index_ex(&p, stream, &sc->phase[r]);
+        if (st != LVSA_OK) { lvsa_schedule_destroy(sc); return st; }
+    }
+    // one-time kernel attribute setup now, so that later launches are pure launches (graph capture)
+    lvsa_status_t st = lvsa_attn_prepare(sc->phase[0]);
+    if (st != LVSA_OK) { lvsa_schedule_destroy(sc); return st; }
+    *out = sc;
+    return LVSA_OK;
+}
+
+int lvsa_schedule_num_phases(const lvsa_schedule_t *sc) { return sc == nullptr ? 0 : sc->n_phases; }
+
+const lvsa_index_t *lvsa_schedule_index(const lvsa_schedule_t *sc, int step) {
+    if (sc == nullptr || step < 0) { lvsa_set_error("NULL schedule or negative step"); return nullptr; }
+    return sc->phase[step % sc->n_phases];
+}
+
+lvsa_status_t lvsa_schedule_attn_fwd(const lvsa_schedule_t *sc, int step, const void *q, const void *k,
+                                     const void *v, void *out, float *lse, void *stream) {
+    const lvsa_index_t *ix = lvsa_schedule_index(sc, step);
+    if (ix == nullptr) return LVSA_EINVAL;
+    return lvsa_attn_fwd(q, k, v, ix, out, lse, stream);
+}
+
+void lvsa_schedule_destroy(lvsa_schedule_t *sc) {
+    if (sc == nullptr) return;
+    if (sc->phase != nullptr) {
+        for (int r = 0; r < sc->n_phases; ++r) lvsa_index_destroy(sc->phase[r]);
+        delete[] sc->phase;
+    }
+    delete sc;
 }
 
 int lvsa_attn_fwd_launches(const lvsa_index_t *ix) { return ix == nullptr ? 0 : 1; }

@@ -17,7 +17,7 @@ __device__ __forceinline__ bool bit_test(const uint32_t *bits, int x) {
 }
 
 // One block.  g_bits lives in shared memory; every thread then owns frames t, t+blockDim, ...
-__global__ void lvsa_frames_kernel(int T, int W, int a, int s, int tie_hi, int words,
+__global__ void lvsa_frames_kernel(int T, int W, int a, int s, int tie_hi, int k0, int has_text, int words,
                                    int32_t *__restrict__ w_lo, int32_t *__restrict__ w_hi,
                                    uint32_t *__restrict__ a_bits, int32_t *__restrict__ meta) {
     extern __shared__ uint32_t g_bits[];
@@ -36,6 +36,9 @@ __global__ void lvsa_frames_kernel(int T, int W, int a, int s, int tie_hi, int w
             atomicOr(&g_bits[f >> 5], 1u << (f & 31));
         }
     }
+    // dedicated initial anchors: frames 0..k0-1 are global at every step (R22)
+    if (!all_tiles)
+        for (int f = tid; f < min(k0, T); f += blockDim.x) atomicOr(&g_bits[f >> 5], 1u << (f & 31));
     __syncthreads();
     if (tid == 0) {
         int c = 0;
@@ -74,15 +77,24 @@ __global__ void lvsa_frames_kernel(int T, int W, int a, int s, int tie_hi, int w
                 const int n = b1 - b0 + 1;
                 rm = (n == 32 ? 0xffffffffu : ((1u << n) - 1u)) << (b0 - 32 * w);
             }
-            a_bits[(size_t)t * words + w] = g_bits[w] | rm;
+            uint32_t bits = g_bits[w] | rm;
+            // text pseudo-frame T (R23): every video query attends to the text tokens
+            if (has_text && (T >> 5) == w) bits |= 1u << (T & 31);
+            a_bits[(size_t)t * words + w] = bits;
         }
     }
+    // ... and the text tokens attend to every frame, themselves included: row T = bits 0..T
+    if (has_text)
+        for (int w = tid; w < words; w += blockDim.x) {
+            const int n = min(32, T + 1 - 32 * w);
+            a_bits[(size_t)T * words + w] = n <= 0 ? 0u : (n == 32 ? 0xffffffffu : ((1u << n) - 1u));
+        }
 }
 
 // One block per q tile; threads stride over kv tiles in ascending chunks so the fill pass can
 // write in order.  FILL = false: counts[i].  FILL = true: indices/flags at indptr[i].
 template <bool FILL>
-__global__ void lvsa_tiles_kernel(long long N, int P, int Bq, int Bk, int nk, int words,
+__global__ void lvsa_tiles_kernel(long long N, int P, int Tf, int Bq, int Bk, int nk, int words,
                                   const uint32_t *__restrict__ a_bits,
                                   const int32_t *__restrict__ indptr, int32_t *__restrict__ counts,
                                   int32_t *__restrict__ indices, uint8_t *__restrict__ flags,
@@ -93,7 +105,8 @@ __global__ void lvsa_tiles_kernel(long long N, int P, int Bq, int Bk, int nk, in
     const int nwarps = blockDim.x >> 5;
     const long long r0 = (long long)i * Bq;
     const long long r1 = min(r0 + Bq, N) - 1;
-    const int f0 = (int)(r0 / P), f1 = (int)(r1 / P);
+    // frame of a token: n / P, tokens past the video (text, R23) belong to the last frame row Tf-1
+    const int f0 = min((int)(r0 / P), Tf - 1), f1 = min((int)(r1 / P), Tf - 1);
     int running = 0, n_part = 0;
     if (FILL && meta[7]) return;   // allocation bound exceeded (reported by the host)
     const int base = FILL ? indptr[i] : 0;
@@ -103,7 +116,7 @@ __global__ void lvsa_tiles_kernel(long long N, int P, int Bq, int Bk, int nk, in
         if (j < nk) {
             const long long c0 = (long long)j * Bk;
             const long long c1 = min(c0 + Bk, N) - 1;
-            const int g0 = (int)(c0 / P), g1 = (int)(c1 / P);
+            const int g0 = min((int)(c0 / P), Tf - 1), g1 = min((int)(c1 / P), Tf - 1);
             part = (c0 + Bk > N);  // columns >= N are never allowed
             for (int tq = f0; tq <= f1; ++tq) {
                 const uint32_t *row = a_bits + (size_t)tq * words;
@@ -218,13 +231,18 @@ lvsa_status_t lvsa_index_build_device(lvsa_index *ix, cudaStream_t stream) {
         if (p.anchors == 0) m_bound = 0;
         else { const long long T_per = (T + p.anchors - 1) / p.anchors; m_bound = (T + T_per - 1) / T_per; }
     }
+    m_bound += p.initial_anchors;
     long long a_bound = m_bound + 2ll * W + 1; if (a_bound > T) a_bound = T;
     const long long fq = (p.tile_q - 1) / p.P + 2, kf = (p.P - 1) / p.tile_k + 2;
-    long long per_q = fq * a_bound * kf; if (per_q > ix->nk) per_q = ix->nk;
+    long long per_q = fq * a_bound * kf;
+    if (p.n_text > 0) per_q += (p.n_text - 1) / p.tile_k + 2;      // the text columns every row keeps
+    if (per_q > ix->nk) per_q = ix->nk;
     ix->n_items = (ix->nq + ix->group - 1) / ix->group;
     long long per_item = per_q * ix->group; if (per_item > ix->nk) per_item = ix->nk;
-    ix->cap_nnz = per_q * ix->nq;
-    ix->cap_item_tiles = per_item * ix->n_items;
+    // q tiles that hold text rows keep every kv tile
+    const long long text_q = p.n_text > 0 ? (p.n_text - 1) / p.tile_q + 2 : 0;
+    ix->cap_nnz = per_q * ix->nq + text_q * ix->nk;
+    ix->cap_item_tiles = per_item * ix->n_items + text_q * ix->nk;
     if (ix->cap_nnz >= (1ll << 31) || ix->cap_item_tiles >= (1ll << 31)) {
         lvsa_set_error("index too large for int32 offsets");
         return LVSA_EUNSUPPORTED;
@@ -234,7 +252,7 @@ lvsa_status_t lvsa_index_build_device(lvsa_index *ix, cudaStream_t stream) {
     size_t off = 0;
     auto take = [&](size_t bytes) { const size_t o = off; off += align_up(bytes); return o; };
     const size_t o_wlo = take(sizeof(int32_t) * T), o_whi = take(sizeof(int32_t) * T);
-    const size_t o_abits = take(sizeof(uint32_t) * (size_t)T * words), o_meta = take(sizeof(int32_t) * 8);
+    const size_t o_abits = take(sizeof(uint32_t) * (size_t)ix->Tf * words), o_meta = take(sizeof(int32_t) * 8);
     const size_t o_indptr = take(sizeof(int32_t) * ((size_t)ix->nq + 1));
     const size_t o_counts = take(sizeof(int32_t) * n_counts);
     const size_t o_indices = take(sizeof(int32_t) * (size_t)(ix->cap_nnz + 1));
@@ -264,15 +282,15 @@ lvsa_status_t lvsa_index_build_device(lvsa_index *ix, cudaStream_t stream) {
 
     LVSA_CUDA_TRY(cudaMemsetAsync(ix->d_meta, 0, sizeof(int32_t) * 8, stream));
     lvsa_frames_kernel<<<1, 256, sizeof(uint32_t) * words, stream>>>(
-        T, W, p.anchors, p.step, p.tie_break == LVSA_TIE_HI, words, ix->d_wlo, ix->d_whi,
+        T, W, p.anchors, p.step, p.tie_break == LVSA_TIE_HI, p.initial_anchors, p.n_text > 0, words, ix->d_wlo, ix->d_whi,
         ix->d_abits, ix->d_meta);
     lvsa_tiles_kernel<false><<<ix->nq, 256, 0, stream>>>(
-        (long long)ix->N, p.P, p.tile_q, p.tile_k, ix->nk, words, ix->d_abits, nullptr, d_counts,
+        (long long)ix->N, p.P, ix->Tf, p.tile_q, p.tile_k, ix->nk, words, ix->d_abits, nullptr, d_counts,
         nullptr, nullptr, ix->d_meta);
     lvsa_scan_kernel<<<1, 1024, 0, stream>>>(d_counts, ix->nq, ix->d_indptr, ix->d_meta + 0,
                                              (long long)ix->cap_nnz, ix->d_meta + 7);
     lvsa_tiles_kernel<true><<<ix->nq, 256, 0, stream>>>(
-        (long long)ix->N, p.P, p.tile_q, p.tile_k, ix->nk, words, ix->d_abits, ix->d_indptr, nullptr,
+        (long long)ix->N, p.P, ix->Tf, p.tile_q, p.tile_k, ix->nk, words, ix->d_abits, ix->d_indptr, nullptr,
         ix->d_indices, ix->d_flags, ix->d_meta);
 
     // work items for the attention kernel

@@ -20,6 +20,7 @@ struct lvsa_index {
     lvsa_params_t p;  // with defaults resolved
     int64_t N = 0;
     int32_t nq = 0, nk = 0, words = 0;
+    int32_t Tf = 0;   // frame rows of A: T video frames (+ 1 text pseudo-frame when n_text > 0, R23)
     // counters computed on the device; fetched lazily (lvsa_index_fetch_meta) so that the build
     // itself never synchronises
     mutable int32_t T_per = 0, phase = 0, n_global = 0;
@@ -73,3 +74,7 @@ int lvsa_attn_sm100_supported(const lvsa_index *ix);
 // lvsa_attn_sm100_ws.cu (warp-specialised persistent kernel, d = 128)
 lvsa_status_t lvsa_attn_sm100_ws_launch(const lvsa_index *ix, const void *q, const void *k,
                                         const void *v, void *out, float *lse, cudaStream_t stream);
+lvsa_status_t lvsa_attn_sm100_ws_prepare(int device);
+
+// lvsa_capi.cu: one-time kernel setup for the index's kernel (used by the schedule driver)
+lvsa_status_t lvsa_attn_prepare(const lvsa_index *ix);

@@ -33,10 +33,12 @@ class Workload:
     layers: tuple = ()    # layers the config asks for
     n_layers: int = 0
     B: int = 1
+    n_text: int = 0       # text tokens after the video tokens (reading R23); 0 = none
+    k0: int = 0           # dedicated initial anchors (reading R22); 0 = the paper's pattern
 
     @property
     def N(self) -> int:
-        return self.T * self.P
+        return self.T * self.P + self.n_text
 
     @property
     def seed(self) -> int:
@@ -59,6 +61,16 @@ WORKLOADS = {
                               steps=tuple(range(10)), layers=(0,), n_layers=4),
     "small128": Workload("small128", 2, T=9, P=200, H=3, d=128, tile=128, W=1, a=2,
                          steps=(0, 1, 2, 3, 4), layers=(0,), n_layers=1),
+    # extension rows: text tokens inside self-attention (f2; the paper's
+    # prompts are "around 500 tokens") and dedicated initial anchors (f3)
+    "tiny_text": Workload("tiny_text", 1, T=8, P=40, H=2, d=64, tile=64, W=1, a=2,
+                          steps=(0, 1, 2, 3), layers=(0,), n_layers=1, n_text=30),
+    "small128_text": Workload("small128_text", 2, T=9, P=200, H=3, d=128, tile=128, W=1, a=2,
+                              steps=(0, 1, 2), layers=(0,), n_layers=1, n_text=77),
+    "small128_k0": Workload("small128_k0", 2, T=9, P=200, H=3, d=128, tile=128, W=1, a=2,
+                            steps=(0, 1, 2), layers=(0,), n_layers=1, k0=2),
+    "hv1.5_1x_text": Workload("hv1.5_1x_text", 5, T=33, P=1590, H=16, d=128, tile=128, W=2, a=12,
+                              steps=(0, 25), layers=(27,), n_layers=54, n_text=512),
 }
 
 
@@ -97,6 +109,8 @@ def sample_rows(w: Workload, n_uniform: int = 3584, n_edge: int = 512,
     edge = {0, N - 1}
     tail0 = (N // tile) * tile if N % tile else N - tile
     edge.update(range(max(tail0, 0), N, max(1, (N - tail0) // 8)))
+    if w.n_text > 0:
+        edge.update((w.T * P - 1, w.T * P))          # last video row, first text row
     ts = rng.permutation(np.arange(1, w.T))
     for t in ts:
         if len(edge) >= n_edge:

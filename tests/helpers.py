@@ -15,7 +15,8 @@ LSE_MAX_ABS_BF16, LSE_MAX_ABS_FP32 = 2e-3, 1e-5
 def build_index(w, step, layer=0, anchors=None, window=None, **kw):
     return binding.lvsa_build_block_index_ex(
         T=w.T, P=w.P, H=w.H, d=w.d, B=w.B, window=w.W if window is None else window,
-        anchors=w.a if anchors is None else anchors, step=step, layer=layer, **kw)
+        anchors=w.a if anchors is None else anchors, step=step, layer=layer,
+        initial_anchors=w.k0, n_text=w.n_text, **kw)
 
 
 def gpu_attn(w, ix, q, k, v, want_lse=True):
@@ -27,9 +28,11 @@ def gpu_attn(w, ix, q, k, v, want_lse=True):
 
 
 def oracle_attn(w, q, k, v, step, rows, anchors=None, window=None, b=0):
-    p = orc.pattern(w.T, w.W if window is None else window, w.a if anchors is None else anchors, step)
+    p = orc.pattern(w.T, w.W if window is None else window, w.a if anchors is None else anchors, step,
+                    initial_anchors=w.k0)
+    A = orc.with_text(p.A) if w.n_text > 0 else p.A
     qa, ka, va = (inputs.to_oracle_array(x[b]) for x in (q, k, v))
-    return orc.attn_rows(qa, ka, va, w.T, w.P, p.A, rows)
+    return orc.attn_rows(qa, ka, va, w.T, w.P, A, rows, n_text=w.n_text)
 
 
 def compare(out_gpu, lse_gpu, out_ref, lse_ref, rows, b=0):

@@ -28,20 +28,24 @@ def test_library_exports_every_declared_symbol():
 
 
 def test_struct_sizes_match_header():
-    # 14 int32 + float; 19 int32 + pad + 5 int64
-    assert C.sizeof(binding.Params) == 15 * 4
-    assert C.sizeof(binding.IndexInfo) == 20 * 4 + 5 * 8
+    # 14 int32 + float + 2 int32; 21 int32 + pad + 5 int64
+    assert C.sizeof(binding.Params) == 17 * 4
+    assert C.sizeof(binding.IndexInfo) == 22 * 4 + 5 * 8
 
 
 def test_argument_validation_needs_no_gpu():
     bad = [dict(T=0, P=4, H=1, d=64), dict(T=4, P=4, H=1, d=64, window=-1),
            dict(T=4, P=4, H=1, d=64, anchors=-2), dict(T=4, P=4, H=1, d=64, step=-1),
            dict(T=4, P=4, H=1, d=64, layer=-1), dict(T=1 << 16, P=1 << 16, H=1, d=64),
-           dict(T=4, P=4, H=1, d=64, tie_break=7)]
+           dict(T=4, P=4, H=1, d=64, tie_break=7), dict(T=4, P=4, H=1, d=64, initial_anchors=-1),
+           dict(T=4, P=4, H=1, d=64, n_text=-1)]
     for kw in bad:
         with pytest.raises(binding.LvsaError) as ei:
             binding.lvsa_build_block_index_ex(**kw)
         assert ei.value.status == binding.EINVAL, kw
+    with pytest.raises(binding.LvsaError) as ei:
+        binding.lvsa_schedule_create(T=4, P=4, H=1, d=64, window=-1)
+    assert ei.value.status == binding.EINVAL
     for kw in [dict(T=4, P=4, H=1, d=96), dict(T=4, P=4, H=1, d=128, tile_q=64, tile_k=64),
                dict(T=4, P=4, H=1, d=64, dtype=binding.DTYPE_FP32, kernel=binding.KERNEL_TCGEN05)]:
         with pytest.raises(binding.LvsaError) as ei:

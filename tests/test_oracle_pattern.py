@@ -251,3 +251,37 @@ def test_alg1_loop_statistics_report_only():
             it = orc.pattern(T, 2, 16, s).iters
             tot += int(it.sum()); calls += T; mx = max(mx, int(it.max()))
     assert abs(tot / calls - 1.21) < 0.01 and mx <= 8
+
+
+# ---------------------------------------------------------------- dedicated initial anchors (R22)
+def test_initial_anchor_golden():
+    # hand-derived example, PAPER.md:54, :58 + Algorithm 1 with G' = G^s u {0..k0-1}
+    for (s, t), want in read_golden_sets("initial_anchor_example_T8_W1_a2_k1.txt"):
+        p = orc.pattern(8, 1, 2, s, initial_anchors=1)
+        assert members(p.A[t]) == want, (s, t)
+
+
+def test_initial_anchors_invariants():
+    for T, W, a in SWEEP:
+        for k0 in (0, 1, 2, 5, T, T + 3):
+            for s in (0, 1, 7):
+                p = orc.pattern(T, W, a, s, initial_anchors=k0)
+                base = orc.pattern(T, W, a, s)
+                if k0 == 0:
+                    # the paper's pattern is the special case k0 = 0
+                    assert np.array_equal(p.A, base.A) and p.n_global == base.n_global
+                # G' = G^s u {0..k0-1}, with G^s restated here from Eq. 3
+                G = set()
+                if a > 0:
+                    T_per = math.ceil(T / a)
+                    G = {((s % T_per) + i * T_per) % T for i in range(math.ceil(T / T_per))}
+                Gp = G | set(range(min(k0, T)))
+                assert members(p.inG) == frozenset(Gp) and p.n_global == len(Gp)
+                # every query frame attends to the dedicated anchors
+                assert p.A[:, :min(k0, T)].all()
+                # closed-form budget with |G'|
+                want = len(Gp) + min(2 * W + 1, T - len(Gp))
+                assert (p.A.sum(1) == want).all(), (T, W, a, k0, s)
+                assert all(p.A[t, t] for t in range(T))
+                if k0 >= T:
+                    assert p.A.all()     # every frame an anchor: dense (Def. 1)
