@@ -192,7 +192,7 @@ def run_ours(args):
     barrier()
     clocks = sampler.stop() if rank == 0 else None
     total_ms = e0.elapsed_time(e1)
-    launches_per_step = 7 + attn_launches   # 7 index-builder kernels + attention
+    launches_per_step = 4 + attn_launches   # 4 index-builder kernels + attention
     step_nnz = [nnz_of[steps_cycle[i % len(steps_cycle)]] for i in range(args.steps)]
     tile_flops = sum(float(n) * w.H * w.B * 4.0 * w.tile * w.tile * w.d for n in step_nnz)
     nnz_mean = float(np.mean(step_nnz))
@@ -214,7 +214,7 @@ def run_ours(args):
         burst.append(k0.elapsed_time(k1))
     burst_ms = float(min(burst))
 
-    # ---- index build alone (a1-a5): 7 kernels, enqueue only; device time by events, host time by clock
+    # ---- index build alone (a1-a5): 4 kernels, enqueue only; device time by events, host time by clock
     torch.cuda.synchronize()
     nb = 20
     b0, b1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)

@@ -94,7 +94,7 @@ typedef struct lvsa_index_info {
  * A kv tile is kept iff some (valid query row, valid key column) pair is allowed; it is PARTIAL
  * iff some (valid row, column of the tile) pair is not (frame not attended, or column >= N).
  * All arithmetic is integer and runs in CUDA kernels on the current device's default stream.
- * The call only ENQUEUES the seven builder kernels and returns: it never synchronises.  Device
+ * The call only ENQUEUES the four builder kernels and returns: it never synchronises.  Device
  * buffers come from one stream-ordered allocation sized by an upper bound on nnz (no device
  * round trip); the counters (nnz, ...) are read back lazily by lvsa_index_info /
  * lvsa_index_copy_host, which do synchronise.  Use the index on the stream it was built on (or

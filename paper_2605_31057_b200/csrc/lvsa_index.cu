@@ -1,10 +1,10 @@
 // GPU index builder: steps a1-a5 of the hot path.
 //   lvsa_frames_kernel : T_per, G^s (Eq. 3), adaptive window,
 //                        Algorithm 1, A(t) bitsets (Def. 2)
-//   lvsa_tiles_kernel  : frame -> token -> tile mapping, count then fill (CSR + FULL/PARTIAL)
-//   lvsa_scan_kernel   : exclusive scan of the per-tile counts
-//   lvsa_items_kernel  : merges the lists of adjacent q tiles into the attention kernel's
-//                        work items (q-tile groups that share K/V loads)
+//   lvsa_tiles_kernel  : frame -> token -> tile mapping per pair of adjacent q tiles, count then
+//                        fill: the CSR (indices + FULL/PARTIAL flags per q tile) and the attention
+//                        kernel's work items (union list of the pair, which shares K/V loads)
+//   lvsa_scan_kernel   : exclusive scans of the per-q-tile and per-item counts (one launch)
 // Integer arithmetic only.  Written from the paper; shares nothing with oracle/.
 #include <limits.h>
 
@@ -91,68 +91,110 @@ __global__ void lvsa_frames_kernel(int T, int W, int a, int s, int tie_hi, int k
         }
 }
 
-// One block per q tile; threads stride over kv tiles in ascending chunks so the fill pass can
-// write in order.  FILL = false: counts[i].  FILL = true: indices/flags at indptr[i].
+// One block per work item = group of two adjacent q tiles (the 256 query rows that share K/V
+// loads in the attention kernel).  Threads stride over kv tiles in ascending chunks, so the fill
+// pass writes in order.  For every kv tile the thread decides kept / PARTIAL for each of the two
+// q tiles (frame -> token -> tile mapping, reading R14); the item's list is the union, each
+// entry tagged with the per-q-tile state (skip / full / partial).
+//   FILL = false: counts[i] per q tile, icounts[g] per item.
+//   FILL = true : indices/flags at indptr[i] (the CSR), item_tiles at item_ptr[g].
 template <bool FILL>
-__global__ void lvsa_tiles_kernel(long long N, int P, int Tf, int Bq, int Bk, int nk, int words,
+__global__ void lvsa_tiles_kernel(long long N, int P, int Tf, int Bq, int Bk, int nq, int nk, int words,
                                   const uint32_t *__restrict__ a_bits,
-                                  const int32_t *__restrict__ indptr, int32_t *__restrict__ counts,
+                                  const int32_t *__restrict__ indptr, const int32_t *__restrict__ item_ptr,
+                                  int32_t *__restrict__ counts, int32_t *__restrict__ icounts,
                                   int32_t *__restrict__ indices, uint8_t *__restrict__ flags,
-                                  int32_t *__restrict__ meta) {
-    __shared__ int warp_tot[32];
-    __shared__ int chunk_base;
-    const int i = blockIdx.x, tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+                                  int32_t *__restrict__ item_tiles, int32_t *__restrict__ meta) {
+    __shared__ int warp_tot[3][32];
+    const int g = blockIdx.x, tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int nwarps = blockDim.x >> 5;
-    const long long r0 = (long long)i * Bq;
-    const long long r1 = min(r0 + Bq, N) - 1;
-    // frame of a token: n / P, tokens past the video (text, R23) belong to the last frame row Tf-1
-    const int f0 = min((int)(r0 / P), Tf - 1), f1 = min((int)(r1 / P), Tf - 1);
-    int running = 0, n_part = 0;
     if (FILL && meta[7]) return;   // allocation bound exceeded (reported by the host)
-    const int base = FILL ? indptr[i] : 0;
+    // rows and frames of the two q tiles; frame of a token: n / P, tokens past the video (text,
+    // R23) belong to the last frame row Tf-1
+    const int i0 = 2 * g, i1 = 2 * g + 1;
+    const bool has1 = i1 < nq;
+    int fa[2], fb[2];
+#pragma unroll
+    for (int w = 0; w < 2; ++w) {
+        const long long r0 = (long long)(i0 + w) * Bq;
+        const long long r1 = min(r0 + Bq, N) - 1;
+        fa[w] = min((int)(r0 / P), Tf - 1);
+        fb[w] = (w == 0 || has1) ? min((int)(r1 / P), Tf - 1) : fa[w] - 1;   // empty range: no q tile 1
+    }
+    int run[3] = {0, 0, 0}, n_part = 0;
+    int base[3] = {0, 0, 0};
+    if (FILL) { base[0] = indptr[i0]; base[1] = has1 ? indptr[i1] : 0; base[2] = item_ptr[g]; }
     for (int j0 = 0; j0 < nk; j0 += blockDim.x) {
         const int j = j0 + tid;
-        bool kept = false, part = false;
+        bool kept[2] = {false, false}, part[2] = {false, false};
         if (j < nk) {
             const long long c0 = (long long)j * Bk;
             const long long c1 = min(c0 + Bk, N) - 1;
             const int g0 = min((int)(c0 / P), Tf - 1), g1 = min((int)(c1 / P), Tf - 1);
-            part = (c0 + Bk > N);  // columns >= N are never allowed
-            for (int tq = f0; tq <= f1; ++tq) {
-                const uint32_t *row = a_bits + (size_t)tq * words;
-                for (int tk = g0; tk <= g1; ++tk) {
-                    const bool b = bit_test(row, tk);
-                    kept |= b; part |= !b;
+            const bool tail = (c0 + Bk > N);  // columns >= N are never allowed
+#pragma unroll
+            for (int w = 0; w < 2; ++w) {
+                part[w] = tail;
+                for (int tq = fa[w]; tq <= fb[w]; ++tq) {
+                    const uint32_t *row = a_bits + (size_t)tq * words;
+                    for (int tk = g0; tk <= g1; ++tk) {
+                        const bool b = bit_test(row, tk);
+                        kept[w] |= b; part[w] |= !b;
+                    }
                 }
             }
         }
-        const unsigned bal = __ballot_sync(0xffffffffu, kept);
-        if (lane == 0) warp_tot[wid] = __popc(bal);
+        const unsigned bal0 = __ballot_sync(0xffffffffu, kept[0]);
+        const unsigned bal1 = __ballot_sync(0xffffffffu, kept[1]);
+        const unsigned balu = bal0 | bal1;
+        if (lane == 0) { warp_tot[0][wid] = __popc(bal0); warp_tot[1][wid] = __popc(bal1); warp_tot[2][wid] = __popc(balu); }
         __syncthreads();
-        int woff = 0, tot = 0;
-        for (int w = 0; w < nwarps; ++w) { const int c = warp_tot[w]; if (w < wid) woff += c; tot += c; }
-        if (FILL && kept) {
-            const int pos = base + running + woff + __popc(bal & ((1u << lane) - 1u));
-            indices[pos] = j;
-            flags[pos] = part ? LVSA_TILE_PARTIAL : LVSA_TILE_FULL;
-            n_part += part;
+        int woff[3] = {0, 0, 0}, tot[3] = {0, 0, 0};
+        for (int w = 0; w < nwarps; ++w)
+#pragma unroll
+            for (int x = 0; x < 3; ++x) { const int c = warp_tot[x][w]; if (w < wid) woff[x] += c; tot[x] += c; }
+        if (FILL) {
+            const unsigned below = (1u << lane) - 1u;
+            if (kept[0]) {
+                const int pos = base[0] + run[0] + woff[0] + __popc(bal0 & below);
+                indices[pos] = j; flags[pos] = part[0] ? LVSA_TILE_PARTIAL : LVSA_TILE_FULL; n_part += part[0];
+            }
+            if (kept[1]) {
+                const int pos = base[1] + run[1] + woff[1] + __popc(bal1 & below);
+                indices[pos] = j; flags[pos] = part[1] ? LVSA_TILE_PARTIAL : LVSA_TILE_FULL; n_part += part[1];
+            }
+            if (kept[0] || kept[1]) {
+                const int st0 = kept[0] ? (part[0] ? LVSA_ST_PARTIAL : LVSA_ST_FULL) : LVSA_ST_SKIP;
+                const int st1 = kept[1] ? (part[1] ? LVSA_ST_PARTIAL : LVSA_ST_FULL) : LVSA_ST_SKIP;
+                item_tiles[base[2] + run[2] + woff[2] + __popc(balu & below)] =
+                    j | (st0 << LVSA_ITEM_J_BITS) | (st1 << (LVSA_ITEM_J_BITS + 2));
+            }
         }
-        running += tot;
+#pragma unroll
+        for (int x = 0; x < 3; ++x) run[x] += tot[x];
         __syncthreads();
     }
-    if (!FILL && tid == 0) counts[i] = running;
+    if (!FILL && tid == 0) { counts[i0] = run[0]; if (has1) counts[i1] = run[1]; icounts[g] = run[2]; }
     if (FILL) {
         n_part = __reduce_add_sync(0xffffffffu, n_part);
         if (lane == 0 && n_part) atomicAdd(&meta[1], n_part);
     }
-    (void)chunk_base;
 }
 
 // Single-block exclusive scan: out[0..n] from counts[0..n-1]; total also to *total_out.
 // If the total exceeds `cap` (the host's allocation bound) meta[7] is raised and the fill passes
 // write nothing; the host reports it at the next lvsa_index_info / copy_host.
-__global__ void lvsa_scan_kernel(const int32_t *__restrict__ counts, int n, int32_t *__restrict__ out,
-                                 int32_t *__restrict__ total_out, long long cap, int32_t *__restrict__ overflow) {
+__global__ void lvsa_scan_kernel(const int32_t *__restrict__ counts_a, int n_a, int32_t *__restrict__ out_a,
+                                 int32_t *__restrict__ total_a, long long cap_a,
+                                 const int32_t *__restrict__ counts_b, int n_b, int32_t *__restrict__ out_b,
+                                 int32_t *__restrict__ total_b, long long cap_b,
+                                 int32_t *__restrict__ overflow) {
+    // block 0 scans the per-q-tile counts (-> indptr), block 1 the per-item counts (-> item_ptr)
+    const int32_t *counts = blockIdx.x == 0 ? counts_a : counts_b;
+    const int n = blockIdx.x == 0 ? n_a : n_b;
+    int32_t *out = blockIdx.x == 0 ? out_a : out_b;
+    int32_t *total_out = blockIdx.x == 0 ? total_a : total_b;
+    const long long cap = blockIdx.x == 0 ? cap_a : cap_b;
     __shared__ int warp_tot[32];
     __shared__ int carry_s;
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5, nwarps = blockDim.x >> 5;
@@ -177,35 +219,6 @@ __global__ void lvsa_scan_kernel(const int32_t *__restrict__ counts, int n, int3
         __syncthreads();
     }
     if (tid == 0) { out[n] = carry_s; *total_out = carry_s; if (carry_s > cap) *overflow = 1; }
-}
-
-// One thread per work item: union of the kv-tile lists of `group` (1 or 2) adjacent q tiles,
-// ascending, each entry tagged with the per-q-tile state (skip / full / partial).
-template <bool FILL>
-__global__ void lvsa_items_kernel(int nq, int group, long long n_items,
-                                  const int32_t *__restrict__ indptr,
-                                  const int32_t *__restrict__ indices,
-                                  const uint8_t *__restrict__ flags,
-                                  const int32_t *__restrict__ item_ptr, int32_t *__restrict__ counts,
-                                  int32_t *__restrict__ item_tiles, const int32_t *__restrict__ overflow) {
-    const long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (g >= n_items || *overflow) return;
-    const int i0 = (int)(g * group), i1 = i0 + 1;
-    int a = indptr[i0], ae = indptr[i0 + 1];
-    int b = 0, be = 0;
-    if (group == 2 && i1 < nq) { b = indptr[i1]; be = indptr[i1 + 1]; }
-    int pos = FILL ? item_ptr[g] : 0, cnt = 0;
-    while (a < ae || b < be) {
-        const int ja = (a < ae) ? indices[a] : INT_MAX;
-        const int jb = (b < be) ? indices[b] : INT_MAX;
-        const int j = min(ja, jb);
-        int st0 = LVSA_ST_SKIP, st1 = LVSA_ST_SKIP;
-        if (ja == j) { st0 = flags[a] ? LVSA_ST_PARTIAL : LVSA_ST_FULL; ++a; }
-        if (jb == j) { st1 = flags[b] ? LVSA_ST_PARTIAL : LVSA_ST_FULL; ++b; }
-        if (FILL) item_tiles[pos + cnt] = j | (st0 << LVSA_ITEM_J_BITS) | (st1 << (LVSA_ITEM_J_BITS + 2));
-        ++cnt;
-    }
-    if (!FILL) counts[g] = cnt;
 }
 
 }  // namespace
@@ -248,13 +261,13 @@ lvsa_status_t lvsa_index_build_device(lvsa_index *ix, cudaStream_t stream) {
         return LVSA_EUNSUPPORTED;
     }
 
-    const size_t n_counts = (size_t)(ix->nq > ix->n_items ? ix->nq : ix->n_items) + 1;
     size_t off = 0;
     auto take = [&](size_t bytes) { const size_t o = off; off += align_up(bytes); return o; };
     const size_t o_wlo = take(sizeof(int32_t) * T), o_whi = take(sizeof(int32_t) * T);
     const size_t o_abits = take(sizeof(uint32_t) * (size_t)ix->Tf * words), o_meta = take(sizeof(int32_t) * 8);
     const size_t o_indptr = take(sizeof(int32_t) * ((size_t)ix->nq + 1));
-    const size_t o_counts = take(sizeof(int32_t) * n_counts);
+    const size_t o_counts = take(sizeof(int32_t) * ((size_t)ix->nq + 1));
+    const size_t o_icounts = take(sizeof(int32_t) * ((size_t)ix->n_items + 1));
     const size_t o_indices = take(sizeof(int32_t) * (size_t)(ix->cap_nnz + 1));
     const size_t o_flags = take((size_t)(ix->cap_nnz + 1));
     const size_t o_item_ptr = take(sizeof(int32_t) * ((size_t)ix->n_items + 1));
@@ -276,7 +289,7 @@ lvsa_status_t lvsa_index_build_device(lvsa_index *ix, cudaStream_t stream) {
     ix->d_wlo = (int32_t *)(a + o_wlo); ix->d_whi = (int32_t *)(a + o_whi);
     ix->d_abits = (uint32_t *)(a + o_abits); ix->d_meta = (int32_t *)(a + o_meta);
     ix->d_indptr = (int32_t *)(a + o_indptr);
-    int32_t *d_counts = (int32_t *)(a + o_counts);
+    int32_t *d_counts = (int32_t *)(a + o_counts), *d_icounts = (int32_t *)(a + o_icounts);
     ix->d_indices = (int32_t *)(a + o_indices); ix->d_flags = a + o_flags;
     ix->d_item_ptr = (int32_t *)(a + o_item_ptr); ix->d_item_tiles = (int32_t *)(a + o_item_tiles);
 
@@ -284,25 +297,16 @@ lvsa_status_t lvsa_index_build_device(lvsa_index *ix, cudaStream_t stream) {
     lvsa_frames_kernel<<<1, 256, sizeof(uint32_t) * words, stream>>>(
         T, W, p.anchors, p.step, p.tie_break == LVSA_TIE_HI, p.initial_anchors, p.n_text > 0, words, ix->d_wlo, ix->d_whi,
         ix->d_abits, ix->d_meta);
-    lvsa_tiles_kernel<false><<<ix->nq, 256, 0, stream>>>(
-        (long long)ix->N, p.P, ix->Tf, p.tile_q, p.tile_k, ix->nk, words, ix->d_abits, nullptr, d_counts,
-        nullptr, nullptr, ix->d_meta);
-    lvsa_scan_kernel<<<1, 1024, 0, stream>>>(d_counts, ix->nq, ix->d_indptr, ix->d_meta + 0,
-                                             (long long)ix->cap_nnz, ix->d_meta + 7);
-    lvsa_tiles_kernel<true><<<ix->nq, 256, 0, stream>>>(
-        (long long)ix->N, p.P, ix->Tf, p.tile_q, p.tile_k, ix->nk, words, ix->d_abits, ix->d_indptr, nullptr,
-        ix->d_indices, ix->d_flags, ix->d_meta);
-
-    // work items for the attention kernel
-    const int ib = 128, ig = (int)((ix->n_items + ib - 1) / ib);
-    lvsa_items_kernel<false><<<ig, ib, 0, stream>>>(ix->nq, ix->group, (long long)ix->n_items,
-                                                     ix->d_indptr, ix->d_indices, ix->d_flags,
-                                                     nullptr, d_counts, nullptr, ix->d_meta + 7);
-    lvsa_scan_kernel<<<1, 1024, 0, stream>>>(d_counts, (int)ix->n_items, ix->d_item_ptr,
-                                             ix->d_meta + 2, (long long)ix->cap_item_tiles, ix->d_meta + 7);
-    lvsa_items_kernel<true><<<ig, ib, 0, stream>>>(ix->nq, ix->group, (long long)ix->n_items,
-                                                    ix->d_indptr, ix->d_indices, ix->d_flags,
-                                                    ix->d_item_ptr, nullptr, ix->d_item_tiles, ix->d_meta + 7);
+    const int n_items = (int)ix->n_items;
+    lvsa_tiles_kernel<false><<<n_items, 256, 0, stream>>>(
+        (long long)ix->N, p.P, ix->Tf, p.tile_q, p.tile_k, ix->nq, ix->nk, words, ix->d_abits, nullptr, nullptr,
+        d_counts, d_icounts, nullptr, nullptr, nullptr, ix->d_meta);
+    lvsa_scan_kernel<<<2, 1024, 0, stream>>>(d_counts, ix->nq, ix->d_indptr, ix->d_meta + 0, (long long)ix->cap_nnz,
+                                             d_icounts, n_items, ix->d_item_ptr, ix->d_meta + 2,
+                                             (long long)ix->cap_item_tiles, ix->d_meta + 7);
+    lvsa_tiles_kernel<true><<<n_items, 256, 0, stream>>>(
+        (long long)ix->N, p.P, ix->Tf, p.tile_q, p.tile_k, ix->nq, ix->nk, words, ix->d_abits, ix->d_indptr,
+        ix->d_item_ptr, nullptr, nullptr, ix->d_indices, ix->d_flags, ix->d_item_tiles, ix->d_meta);
     LVSA_CUDA_TRY(cudaGetLastError());
     ix->meta_fetched = false;
     return LVSA_OK;
