@@ -26,7 +26,12 @@
  * softmax(QK^T/sqrt d)V, per-frame gathered SDPA,
  * rows summing to 1, the Q=0 closed form, token-level N x N brute force on tiny
  * inputs.  Parity UNPINNED (fixed by DESIGN.md readings, not by the paper):
- * the default W (R1), HunyuanVideo's C (R2), the Algorithm-1 tie-break (R5).
+ * the default W (R1), HunyuanVideo's C (R2), the Algorithm-1 tie-break (R5), and the two
+ * extension rules the paper names without specifying: dedicated initial anchors (R22,
+ * lvsa_oracle_pattern_ex) and text tokens inside self-attention (R23, frame_of;
+ * PAPER.md:132).  Their pins (tests/test_oracle_extensions.py, test_oracle_pattern.py) check that
+ * the oracle computes exactly the stated rule: a hand-derived golden example, closed-form budgets,
+ * a token-level N x N numpy mask and library SDPA on gathered keys.
  */
 #include <math.h>
 #include <stdint.h>
