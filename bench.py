@@ -225,6 +225,10 @@ def run_ours(args):
     sched_line = None
     if rank == 0 and not args.no_schedule:
         torch.cuda.synchronize()
+        # warm-up: the first creation grows the stream-ordered pool by T_per arenas (milliseconds)
+        binding.lvsa_schedule_create(stream=stream.cuda_stream, T=w.T, P=w.P, H=w.H, d=w.d, B=w.B,
+                                     window=w.W, anchors=w.a).destroy()
+        torch.cuda.synchronize()
         c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         c0.record(stream)
         sched = binding.lvsa_schedule_create(stream=stream.cuda_stream, T=w.T, P=w.P, H=w.H, d=w.d, B=w.B,
