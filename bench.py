@@ -350,7 +350,7 @@ def run_ours(args):
                          "unit": "TFLOP/s", "frac": round(achieved / peak_sus, 4), "traffic": traffic,
                          "peak_source": pk["_source"] + " bf16 SUSTAINED peak: the kernel is timed inside the "
                                         "long step (event pair around each of the %d launches)" % args.steps,
-                         "kernel": "lvsa_attn_sm100_ws_kernel", "flops_per_launch": kern_flops,
+                         "kernel": "lvsa_attn_sm100_pair_kernel", "flops_per_launch": kern_flops,
                          "ms_per_launch": round(kern_ms, 4),
                          "traffic_source": traffic_src,
                          "burst": {"ms_per_launch": round(burst_ms, 4), "achieved": round(burst_tf, 2),

@@ -359,6 +359,9 @@ lvsa_status_t lvsa_attn_sm100_launch(const lvsa_index *ix, const void *q, const 
         // LVSA_SM100_V0=1 selects the bring-up kernel (debugging aid; same results)
         static const bool force_v0 = getenv("LVSA_SM100_V0") != nullptr && getenv("LVSA_SM100_V0")[0] == '1';
         if (force_v0 || g_dbg != nullptr) return launch_v0<128, 128>(ix, q, k, v, out, lse, stream);
+        // LVSA_PAIR=0 selects the one-CTA warp-specialised kernel (A/B timing; same results)
+        static const bool no_pair = getenv("LVSA_PAIR") != nullptr && getenv("LVSA_PAIR")[0] == '0';
+        if (!no_pair) return lvsa_attn_sm100_pair_launch(ix, q, k, v, out, lse, stream);
         return lvsa_attn_sm100_ws_launch(ix, q, k, v, out, lse, stream);
     }
     return launch_v0<64, 64>(ix, q, k, v, out, lse, stream);

@@ -29,7 +29,10 @@ static int use_tcgen05(const lvsa_index *ix) {
 }
 
 lvsa_status_t lvsa_attn_prepare(const lvsa_index *ix) {
-    if (use_tcgen05(ix) && ix->p.d == 128) return lvsa_attn_sm100_ws_prepare(ix->device);
+    if (use_tcgen05(ix) && ix->p.d == 128) {
+        lvsa_status_t st = lvsa_attn_sm100_pair_prepare(ix->device);
+        return st != LVSA_OK ? st : lvsa_attn_sm100_ws_prepare(ix->device);
+    }
     return LVSA_OK;   // the other kernels set their attributes at launch
 }
 
@@ -38,7 +41,7 @@ extern "C" {
 const char *lvsa_last_error(void) { return g_last_error.c_str(); }
 
 const char *lvsa_version(void) {
-    return "liblvsa 0.1 (sm_100a; kernels: index-builder, attn-simt-fp32, attn-tcgen05-bf16)";
+    return "liblvsa 0.1 (sm_100a; kernels: index-builder, attn-simt-fp32, attn-tcgen05-bf16 (CTA-pair cta_group::2, one-CTA warp-specialised, v0))";
 }
 
 lvsa_status_t lvsa_build_block_index_ex(const lvsa_params_t *params, void *stream, lvsa_index_t **out) {

@@ -76,5 +76,10 @@ lvsa_status_t lvsa_attn_sm100_ws_launch(const lvsa_index *ix, const void *q, con
                                         const void *v, void *out, float *lse, cudaStream_t stream);
 lvsa_status_t lvsa_attn_sm100_ws_prepare(int device);
 
+// lvsa_attn_sm100_pair.cu (CTA-pair kernel, cta_group::2, d = 128)
+lvsa_status_t lvsa_attn_sm100_pair_launch(const lvsa_index *ix, const void *q, const void *k,
+                                          const void *v, void *out, float *lse, cudaStream_t stream);
+lvsa_status_t lvsa_attn_sm100_pair_prepare(int device);
+
 // lvsa_capi.cu: one-time kernel setup for the index's kernel (used by the schedule driver)
 lvsa_status_t lvsa_attn_prepare(const lvsa_index *ix);

@@ -66,6 +66,7 @@ def test_edge_shapes(kname):
              W("odd_nq", 1, T=3, P=128, H=1, d=128, tile=128, W=0, a=1),            # nq = 3: lone last q tile
              W("tiny_frames", 1, T=40, P=7, H=1, d=64, tile=64, W=1, a=3),          # many frames per tile
              W("batch2", 1, T=6, P=70, H=2, d=64, tile=64, W=1, a=2, B=2),
+             W("batch2_d128", 1, T=5, P=150, H=2, d=128, tile=128, W=1, a=2, B=2),  # pair kernel, odd nq, B = 2
              W("dense_window", 1, T=5, P=90, H=2, d=128, tile=128, W=2, a=0),       # 2W+1 >= T: Eq. 1
              W("all_anchors", 1, T=6, P=60, H=1, d=64, tile=64, W=0, a=6)]
     for w in cases:
