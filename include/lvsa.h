@@ -131,6 +131,10 @@ lvsa_status_t lvsa_attn_fwd(const void *q, const void *k, const void *v,
  * a device workspace owned by the library (one per process, allocated on first use, grown on
  * demand, shared by all indices; freed by lvsa_workspace_release), runs lvsa_attn_fwd on
  * `stream`, copies out (and lse if not NULL) back, and synchronises `stream` before returning.
+ * With the CTA-pair kernel (bf16, d = 128) the call is pipelined over groups of heads (by default one
+ * head per group, at most 16 groups; LVSA_HOST_GROUPS overrides): the host-to-device copy of the next group and the
+ * device-to-host copy of the previous one run on two internal streams while the kernel of the
+ * current group runs on `stream`.  Results are identical to the unpipelined call.
  * Calls through the workspace are serialised by a mutex.
  */
 lvsa_status_t lvsa_attn_fwd_host(const void *q_host, const void *k_host, const void *v_host,

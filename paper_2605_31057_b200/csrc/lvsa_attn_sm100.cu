@@ -349,6 +349,17 @@ int lvsa_attn_sm100_supported(const lvsa_index *ix) {
     return (ix->p.d == 128 && ix->p.tile_q == 128) || (ix->p.d == 64 && ix->p.tile_q == 64);
 }
 
+static bool pair_disabled() {
+    // LVSA_PAIR=0 selects the one-CTA warp-specialised kernel (A/B timing; same results)
+    static const bool no_pair = getenv("LVSA_PAIR") != nullptr && getenv("LVSA_PAIR")[0] == '0';
+    return no_pair;
+}
+
+int lvsa_attn_uses_pair_kernel(const lvsa_index *ix) {
+    static const bool force_v0 = getenv("LVSA_SM100_V0") != nullptr && getenv("LVSA_SM100_V0")[0] == '1';
+    return ix->p.d == 128 && !force_v0 && g_dbg == nullptr && !pair_disabled();
+}
+
 lvsa_status_t lvsa_attn_sm100_launch(const lvsa_index *ix, const void *q, const void *k,
                                      const void *v, void *out, float *lse, cudaStream_t stream) {
     if (ix->p.H > 65535 || ix->p.B > 65535) {
@@ -359,9 +370,7 @@ lvsa_status_t lvsa_attn_sm100_launch(const lvsa_index *ix, const void *q, const 
         // LVSA_SM100_V0=1 selects the bring-up kernel (debugging aid; same results)
         static const bool force_v0 = getenv("LVSA_SM100_V0") != nullptr && getenv("LVSA_SM100_V0")[0] == '1';
         if (force_v0 || g_dbg != nullptr) return launch_v0<128, 128>(ix, q, k, v, out, lse, stream);
-        // LVSA_PAIR=0 selects the one-CTA warp-specialised kernel (A/B timing; same results)
-        static const bool no_pair = getenv("LVSA_PAIR") != nullptr && getenv("LVSA_PAIR")[0] == '0';
-        if (!no_pair) return lvsa_attn_sm100_pair_launch(ix, q, k, v, out, lse, stream);
+        if (!pair_disabled()) return lvsa_attn_sm100_pair_launch(ix, q, k, v, out, lse, stream);
         return lvsa_attn_sm100_ws_launch(ix, q, k, v, out, lse, stream);
     }
     return launch_v0<64, 64>(ix, q, k, v, out, lse, stream);

@@ -81,7 +81,7 @@ lvsa_attn_sm100_pair_kernel(const __grid_constant__ CUtensorMap tmap_q,
                             __nv_bfloat16 *__restrict__ out, float *__restrict__ lse,
                             const int32_t *__restrict__ item_ptr, const int32_t *__restrict__ item_tiles,
                             const uint32_t *__restrict__ a_bits, int words, long long N, int P, int T,
-                            int H, int n_items, long long n_work, float scale_log2) {
+                            int H, int h0, int hc, int n_items, long long n_work, float scale_log2) {
     using SM = SmemP<NS>;
     extern __shared__ __align__(1024) uint8_t smem_raw[];
     const uint32_t base = smem_u32(smem_raw);
@@ -144,7 +144,7 @@ lvsa_attn_sm100_pair_kernel(const __grid_constant__ CUtensorMap tmap_q,
         uint32_t oc = 0;            // items finished
         for (long long work = pair; work < n_work; work += n_pairs) {
             const int item = (int)(work % n_items);
-            const int bh = (int)(work / n_items), h = bh % H, b = bh / H;
+            const int bh = (int)(work / n_items), h = h0 + bh % hc, b = bh / hc;   // heads [h0, h0 + hc) of H
             const long long my_row = (long long)item * 256 + rank * 128 + rw;
             const int fq = (int)min((long long)(T - 1), my_row / P);
             const uint32_t *arow = a_bits + (size_t)fq * words;
@@ -351,7 +351,7 @@ lvsa_attn_sm100_pair_kernel(const __grid_constant__ CUtensorMap tmap_q,
             };
             for (long long work = pair; work < n_work; work += n_pairs) {
                 const int item = (int)(work % n_items);
-                const int bh = (int)(work / n_items), h = bh % H, b = bh / H;
+                const int bh = (int)(work / n_items), h = h0 + bh % hc, b = bh / hc;   // heads [h0, h0 + hc) of H
                 const long long row0 = (long long)item * 256 + (long long)rank * 128;
                 const int e0 = item_ptr[item], e1 = item_ptr[item + 1];
                 mbar_wait(bar(SM::Q_EMPTY), (qi & 1u) ^ 1u);
@@ -478,8 +478,10 @@ lvsa_status_t lvsa_attn_sm100_pair_prepare(int device) {
     return LVSA_OK;
 }
 
-lvsa_status_t lvsa_attn_sm100_pair_launch(const lvsa_index *ix, const void *q, const void *k, const void *v,
-                                          void *out, float *lse, cudaStream_t stream) {
+// Heads [h0, h0 + hc) only (all batches): the host entry point pipelines head groups against the
+// PCIe copies.  q, k, v, out, lse are the FULL tensors.
+lvsa_status_t lvsa_attn_sm100_pair_launch_heads(const lvsa_index *ix, const void *q, const void *k, const void *v,
+                                                void *out, float *lse, int h0, int hc, cudaStream_t stream) {
     constexpr int NS = LVSA_PAIR_STAGES;
     using SM = SmemP<NS>;
     CUtensorMap mq, mk, mv;
@@ -488,13 +490,18 @@ lvsa_status_t lvsa_attn_sm100_pair_launch(const lvsa_index *ix, const void *q, c
     if ((st = lvsa_make_tmap_bf16(&mk, k, ix->N, ix->p.H, D, ix->p.B, 64)) != LVSA_OK) return st;
     if ((st = lvsa_make_tmap_bf16(&mv, v, ix->N, ix->p.H, D, ix->p.B, BT)) != LVSA_OK) return st;
     if ((st = lvsa_attn_sm100_pair_prepare(ix->device)) != LVSA_OK) return st;
-    const long long n_work = (long long)ix->n_items * ix->p.H * ix->p.B;
+    const long long n_work = (long long)ix->n_items * hc * ix->p.B;
     long long n_pairs = g_pair_n_sm / 2;
     if (n_work < n_pairs) n_pairs = n_work;
     const float scale_log2 = ix->p.softmax_scale * 1.4426950408889634f;
     lvsa_attn_sm100_pair_kernel<NS><<<(unsigned)(2 * n_pairs), NTHREADS, SM::BYTES, stream>>>(
         mq, mk, mv, (__nv_bfloat16 *)out, lse, ix->d_item_ptr, ix->d_item_tiles, ix->d_abits, ix->words,
-        (long long)ix->N, ix->p.P, ix->Tf, ix->p.H, (int)ix->n_items, n_work, scale_log2);
+        (long long)ix->N, ix->p.P, ix->Tf, ix->p.H, h0, hc, (int)ix->n_items, n_work, scale_log2);
     LVSA_CUDA_TRY(cudaGetLastError());
     return LVSA_OK;
+}
+
+lvsa_status_t lvsa_attn_sm100_pair_launch(const lvsa_index *ix, const void *q, const void *k, const void *v,
+                                          void *out, float *lse, cudaStream_t stream) {
+    return lvsa_attn_sm100_pair_launch_heads(ix, q, k, v, out, lse, 0, ix->p.H, stream);
 }

@@ -1,5 +1,6 @@
 // C ABI of liblvsa (include/lvsa.h): argument checks, handle lifetime, kernel selection.
 #include <math.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <mutex>
@@ -19,6 +20,24 @@ lvsa_status_t lvsa_cuda_fail(cudaError_t e, const char *what) {
 // staging buffers of lvsa_attn_fwd_host (process-wide, one device at a time)
 static struct { void *ptr = nullptr; size_t cap = 0; int device = -1; } g_ws;
 static std::mutex g_ws_mutex;
+
+// streams and events of the pipelined host entry point (created on first use, process lifetime)
+struct HostPipe {
+    static constexpr int MAXG = 16;
+    cudaStream_t s_in = nullptr, s_out = nullptr;
+    cudaEvent_t ev_in[MAXG] = {}, ev_c[MAXG] = {}, ev_edge = nullptr;
+};
+static HostPipe g_host;
+
+// records that `stream` used the index (its arena is stream-ordered memory)
+static bool index_touch_stream(const lvsa_index *index, cudaStream_t stream) {
+    if (index->last_stream != stream) {
+        index->multi_stream = true;
+        index->last_stream = stream;
+        return true;
+    }
+    return false;
+}
 
 static size_t elem_size(const lvsa_index *ix) { return ix->p.dtype == LVSA_DTYPE_FP32 ? 4 : 2; }
 
@@ -123,11 +142,7 @@ lvsa_status_t lvsa_attn_fwd(const void *q, const void *k, const void *v, const l
         lvsa_set_error("q, k, v, out must be 16-byte aligned");
         return LVSA_EINVAL;
     }
-    if (index->last_stream != (cudaStream_t)stream) {
-        // the arena is stream-ordered memory: remember when it is no longer owned by one stream
-        index->multi_stream = true;
-        index->last_stream = (cudaStream_t)stream;
-    }
+    index_touch_stream(index, (cudaStream_t)stream);   // the arena is stream-ordered memory
     if (use_tcgen05(index)) return lvsa_attn_sm100_launch(index, q, k, v, out, lse, (cudaStream_t)stream);
     return lvsa_attn_simt_launch(index, q, k, v, out, lse, (cudaStream_t)stream);
 }
@@ -154,6 +169,65 @@ lvsa_status_t lvsa_attn_fwd_host(const void *qh, const void *kh, const void *vh,
     uint8_t *wsp = static_cast<uint8_t *>(g_ws.ptr);
     void *s_q = wsp, *s_k = wsp + ab, *s_v = wsp + 2 * ab, *s_o = wsp + 3 * ab;
     float *s_lse = reinterpret_cast<float *>(wsp + 4 * ab);
+    // Pipelined path (CTA-pair kernel, bf16): heads are independent, so the call is cut into groups
+    // of heads; the H2D copy of group g+1 and the D2H copy of group g-1 overlap the kernel of
+    // group g (strided 2-D copies of the [B*N, H*d] matrices, one column block per group).
+    static const int n_groups_env = getenv("LVSA_HOST_GROUPS") != nullptr ? atoi(getenv("LVSA_HOST_GROUPS")) : 16;
+    const int H = ix->p.H;
+    int G = n_groups_env < 1 ? 1 : n_groups_env;
+    if (G > H) G = H;
+    if (G > 1 && use_tcgen05(ix) && lvsa_attn_uses_pair_kernel(ix)) {
+        if (g_host.s_in == nullptr) {
+            LVSA_CUDA_TRY(cudaStreamCreateWithFlags(&g_host.s_in, cudaStreamNonBlocking));
+            LVSA_CUDA_TRY(cudaStreamCreateWithFlags(&g_host.s_out, cudaStreamNonBlocking));
+            for (int i = 0; i < HostPipe::MAXG; ++i) {
+                LVSA_CUDA_TRY(cudaEventCreateWithFlags(&g_host.ev_in[i], cudaEventDisableTiming));
+                LVSA_CUDA_TRY(cudaEventCreateWithFlags(&g_host.ev_c[i], cudaEventDisableTiming));
+            }
+            LVSA_CUDA_TRY(cudaEventCreateWithFlags(&g_host.ev_edge, cudaEventDisableTiming));
+        }
+        if (G > HostPipe::MAXG) G = HostPipe::MAXG;
+        const size_t es = elem_size(ix), row = (size_t)H * ix->p.d * es;     // bytes per token (all heads)
+        const size_t rows = (size_t)ix->p.B * ix->N;
+        const int per = (H + G - 1) / G;
+        index_touch_stream(ix, stream);
+        // copies start after whatever the caller already enqueued on `stream`
+        LVSA_CUDA_TRY(cudaEventRecord(g_host.ev_edge, stream));
+        LVSA_CUDA_TRY(cudaStreamWaitEvent(g_host.s_in, g_host.ev_edge, 0));
+        LVSA_CUDA_TRY(cudaStreamWaitEvent(g_host.s_out, g_host.ev_edge, 0));
+        int ng = 0;
+        for (int h0 = 0; h0 < H; h0 += per, ++ng) {
+            const int hc = h0 + per <= H ? per : H - h0;
+            const size_t off = (size_t)h0 * ix->p.d * es, width = (size_t)hc * ix->p.d * es;
+            const void *src[3] = {qh, kh, vh};
+            void *dst[3] = {s_q, s_k, s_v};
+            for (int t = 0; t < 3; ++t)
+                LVSA_CUDA_TRY(cudaMemcpy2DAsync((uint8_t *)dst[t] + off, row, (const uint8_t *)src[t] + off, row, width,
+                                                rows, cudaMemcpyHostToDevice, g_host.s_in));
+            LVSA_CUDA_TRY(cudaEventRecord(g_host.ev_in[ng], g_host.s_in));
+        }
+        ng = 0;
+        for (int h0 = 0; h0 < H; h0 += per, ++ng) {
+            const int hc = h0 + per <= H ? per : H - h0;
+            const size_t off = (size_t)h0 * ix->p.d * es, width = (size_t)hc * ix->p.d * es;
+            LVSA_CUDA_TRY(cudaStreamWaitEvent(stream, g_host.ev_in[ng], 0));
+            lvsa_status_t st = lvsa_attn_sm100_pair_launch_heads(ix, s_q, s_k, s_v, s_o, s_lse, h0, hc, stream);
+            if (st != LVSA_OK) return st;
+            LVSA_CUDA_TRY(cudaEventRecord(g_host.ev_c[ng], stream));
+            LVSA_CUDA_TRY(cudaStreamWaitEvent(g_host.s_out, g_host.ev_c[ng], 0));
+            LVSA_CUDA_TRY(cudaMemcpy2DAsync((uint8_t *)oh + off, row, (const uint8_t *)s_o + off, row, width, rows,
+                                            cudaMemcpyDeviceToHost, g_host.s_out));
+            if (lseh != nullptr)   // lse is [B, H, N]: heads h0.. of every batch are contiguous runs of hc * N floats
+                LVSA_CUDA_TRY(cudaMemcpy2DAsync(lseh + (size_t)h0 * ix->N, sizeof(float) * (size_t)H * ix->N,
+                                                s_lse + (size_t)h0 * ix->N, sizeof(float) * (size_t)H * ix->N,
+                                                sizeof(float) * (size_t)hc * ix->N, (size_t)ix->p.B,
+                                                cudaMemcpyDeviceToHost, g_host.s_out));
+        }
+        LVSA_CUDA_TRY(cudaEventRecord(g_host.ev_edge, g_host.s_out));
+        LVSA_CUDA_TRY(cudaStreamWaitEvent(stream, g_host.ev_edge, 0));
+        LVSA_CUDA_TRY(cudaStreamSynchronize(stream));
+        return LVSA_OK;
+    }
     LVSA_CUDA_TRY(cudaMemcpyAsync(s_q, qh, bytes, cudaMemcpyHostToDevice, stream));
     LVSA_CUDA_TRY(cudaMemcpyAsync(s_k, kh, bytes, cudaMemcpyHostToDevice, stream));
     LVSA_CUDA_TRY(cudaMemcpyAsync(s_v, vh, bytes, cudaMemcpyHostToDevice, stream));

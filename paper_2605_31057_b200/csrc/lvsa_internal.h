@@ -79,7 +79,11 @@ lvsa_status_t lvsa_attn_sm100_ws_prepare(int device);
 // lvsa_attn_sm100_pair.cu (CTA-pair kernel, cta_group::2, d = 128)
 lvsa_status_t lvsa_attn_sm100_pair_launch(const lvsa_index *ix, const void *q, const void *k,
                                           const void *v, void *out, float *lse, cudaStream_t stream);
+lvsa_status_t lvsa_attn_sm100_pair_launch_heads(const lvsa_index *ix, const void *q, const void *k,
+                                                const void *v, void *out, float *lse, int h0, int hc,
+                                                cudaStream_t stream);
 lvsa_status_t lvsa_attn_sm100_pair_prepare(int device);
+int lvsa_attn_uses_pair_kernel(const lvsa_index *ix);   // lvsa_attn_sm100.cu
 
 // lvsa_capi.cu: one-time kernel setup for the index's kernel (used by the schedule driver)
 lvsa_status_t lvsa_attn_prepare(const lvsa_index *ix);
