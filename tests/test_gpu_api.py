@@ -106,3 +106,18 @@ def test_attn_fwd_argument_errors():
     assert L.lvsa_schedule_attn_fwd(null, 0, p(q), p(k), p(v), p(out), null, stream) == binding.EINVAL
     ix.destroy()
     ix.destroy()                      # second destroy of the Python wrapper is a no-op
+
+
+def test_repeated_launches_are_bitwise_identical():
+    """The result does not depend on timing: the MMAs of a q tile accumulate in list order and the
+    rescale decisions are taken in tile order, so repeated launches must agree bit for bit (a race in
+    the mbarrier / TMEM / shared-reference protocols would show up here)."""
+    for name, n in (("small128", 40), ("wan1.3b_1x", 25)):
+        w = inputs.WORKLOADS[name]
+        q, k, v = inputs.make_qkv(w, "cuda", torch.bfloat16)
+        ix = build_index(w, w.steps[0])
+        ref, ref_lse = gpu_attn(w, ix, q, k, v)
+        for _ in range(n):
+            out, lse = gpu_attn(w, ix, q, k, v)
+            assert torch.equal(out, ref) and torch.equal(lse, ref_lse)
+        ix.destroy()
