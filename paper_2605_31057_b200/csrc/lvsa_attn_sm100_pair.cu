@@ -196,8 +196,9 @@ lvsa_attn_sm100_pair_kernel(const __grid_constant__ CUtensorMap tmap_q,
                 }
                 tmem_wait_ld();
 
+                uint32_t cm[4] = {~0u, ~0u, ~0u, ~0u};   // columns of this tile my row may attend to
                 if (st == LVSA_ST_PARTIAL) {
-                    uint32_t cm[4] = {0u, 0u, 0u, 0u};
+                    cm[0] = cm[1] = cm[2] = cm[3] = 0u;
                     const long long col0 = (long long)(entry & LVSA_ITEM_J_MASK) * BT;
                     const long long cend = min(col0 + BT, N);
                     int g = min((int)(col0 / P), T - 1);
@@ -272,7 +273,12 @@ lvsa_attn_sm100_pair_kernel(const __grid_constant__ CUtensorMap tmap_q,
 #pragma unroll
                     for (int c = 0; c < 4; ++c) {
                         uint32_t pk[16];
-                        lvsa_sm::exp_chunk32<0>(s, c * 32, scale2, negm2, pk, lsum);
+                        if (cm[c] == 0u) {   // a fully masked group of 32 columns: P = 0 without the exponentials
+#pragma unroll
+                            for (int x = 0; x < 16; ++x) pk[x] = 0u;
+                        } else {
+                            lvsa_sm::exp_chunk32<0>(s, c * 32, scale2, negm2, pk, lsum);
+                        }
                         tmem_st_32x32b_x16(tS + c * 16, pk);
                         if (c == 1) publish(pa_full);
                     }
