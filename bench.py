@@ -126,6 +126,10 @@ def run_ours(args):
     dev = torch.device("cuda", local)
     torch.cuda.set_device(dev)
     w = inputs.WORKLOADS[args.workload]
+    if args.window is not None or args.anchors is not None:
+        import dataclasses
+        w = dataclasses.replace(w, W=w.W if args.window is None else args.window,
+                                a=w.a if args.anchors is None else args.anchors)
     pk = peaks()
     q, k, v = inputs.make_qkv(w, f"cuda:{local}", torch.bfloat16, seed=w.seed + rank)
     out = torch.empty_like(q)
@@ -319,6 +323,16 @@ def run_ours(args):
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu:
         cpu = cpu_baseline(w, q, k, v, steps_cycle[0], args.cpu_rows)
+        # the same oracle on ONE core (a sixteenth of the sample), and its frame-level mask builder per
+        # denoising step next to the paper's "1.4 us per call, < 200 us per rebuild"
+        one = cpu_baseline(w, q, k, v, steps_cycle[0], max(8, args.cpu_rows // 16), nthreads=1)
+        from oracle import lvsa_oracle as orc
+        sec_rebuild, it_max, it_mean = orc.time_rebuild(w.T, w.W, w.a, 50, reps=20)
+        cpu["one_core"] = {"value": one["value"], "seconds": one["seconds"], "sample": one["sample"]}
+        cpu["mask_builder"] = {"us_per_step_one_core": round(sec_rebuild * 1e6, 2),
+                               "us_per_frame_call": round(sec_rebuild * 1e6 / w.T, 3),
+                               "alg1_loop_max": it_max, "alg1_loop_mean": round(it_mean, 3),
+                               "paper": "1.4 us per call, < 200 us per rebuild, loop <= 8 (mean 1.21), PAPER.md:91"}
 
     if rank == 0:
         peak_sus = pk["bf16_tflops_sustained"]
@@ -430,6 +444,8 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-dense", action="store_true")
     ap.add_argument("--no-schedule", action="store_true")
+    ap.add_argument("--window", type=int, default=None, help="override W of the workload (sensitivity runs)")
+    ap.add_argument("--anchors", type=int, default=None, help="override a = C - (2W+1) of the workload")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.cpu_rows is None:

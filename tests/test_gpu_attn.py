@@ -40,6 +40,9 @@ def run_case(w, kname, steps, rows=None, layer=0, anchors=None, window=None, see
             assert st["nan"] == 0, (kname, s, st)
             assert st["max_abs"] <= mx and st["mean_abs"] <= mean, (kname, s, st)
             assert st["lse_max_abs"] <= lse_tol, (kname, s, st)
+            # |out| is ~0.01 on the large i.i.d. configs, the same order as the max-abs bound, so the
+            # relative error is asserted too (keep it below 2e-2; observed 2e-3)
+            assert st["rel_l2"] <= 2e-2, (kname, s, st)
         ix.destroy()
 
 
