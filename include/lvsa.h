@@ -38,7 +38,14 @@ typedef enum {
 enum { LVSA_TILE_FULL = 0, LVSA_TILE_PARTIAL = 1 };            /* values of flags[]            */
 enum { LVSA_TIE_LO = 0, LVSA_TIE_HI = 1 };                     /* Algorithm 1 line 5 tie-break */
 enum { LVSA_DTYPE_BF16 = 0, LVSA_DTYPE_FP32 = 1 };             /* element type of q,k,v,out    */
-enum { LVSA_KERNEL_AUTO = 0, LVSA_KERNEL_SIMT = 1, LVSA_KERNEL_TCGEN05 = 2 };
+/* LVSA_KERNEL_TCGEN05: the production tensor-core kernel (d = 128: persistent CTA-pair kernel,
+ * cta_group::2; d = 64: the one-CTA-per-item kernel).  LVSA_KERNEL_TCGEN05_V0: the simple
+ * one-CTA-per-item tcgen05 kernel for d = 128 too (a second implementation of the same maths, kept
+ * as an A/B and cross-check variant; same results within the stated tolerance). */
+enum { LVSA_KERNEL_AUTO = 0, LVSA_KERNEL_SIMT = 1, LVSA_KERNEL_TCGEN05 = 2, LVSA_KERNEL_TCGEN05_V0 = 3 };
+/* Memory order of q, k, v, out (PAPER.md:31 fixes only N = T*P, not the order of the axes):
+ * NHD = [B, N, H, d] (default), HND = [B, H, N, d]; d is always fastest.  lse is [B, H, N] in both. */
+enum { LVSA_LAYOUT_NHD = 0, LVSA_LAYOUT_HND = 1 };
 
 /* Parameters of lvsa_build_block_index_ex.  Zero means "default" where a default is named. */
 typedef struct lvsa_params {
@@ -57,13 +64,17 @@ typedef struct lvsa_params {
     int32_t tie_break;  /* LVSA_TIE_LO (default) or LVSA_TIE_HI                                 */
     int32_t dtype;      /* LVSA_DTYPE_BF16 (default, tensor-core kernel) or LVSA_DTYPE_FP32
                            (SIMT kernel only)                                                   */
-    int32_t kernel;     /* LVSA_KERNEL_AUTO: tcgen05 for bf16, SIMT for fp32                    */
+    int32_t kernel;     /* LVSA_KERNEL_AUTO: tcgen05 for bf16, SIMT for fp32; or one of the
+                           LVSA_KERNEL_* values above                                           */
     float softmax_scale;/* default 1/sqrt(d) (Eq. 1)                                            */
     int32_t initial_anchors; /* k0 >= 0 dedicated initial anchors: frames 0..k0-1 join G^s at every
                            step (reading R22).  0 = the paper's pattern */
     int32_t n_text;     /* >= 0 extra tokens after the T*P video tokens (HunyuanVideo's text tokens
                            inside self-attention).  Every query attends to them and they
                            attend to every token (reading R23).  N = T*P + n_text.          */
+    int32_t layout;     /* LVSA_LAYOUT_NHD (default) or LVSA_LAYOUT_HND: memory order of q,k,v,out     */
+    int32_t host_groups;/* lvsa_attn_fwd_host only: number of head groups the call is pipelined over
+                           (0 = default: one head per group, at most 16 groups; 1 = unpipelined)      */
 } lvsa_params_t;
 
 typedef struct lvsa_index_info {
@@ -78,6 +89,7 @@ typedef struct lvsa_index_info {
     int32_t dtype, kernel;
     int32_t n_text;          /* text tokens after the video tokens (R23)                        */
     int32_t initial_anchors; /* dedicated initial anchors k0 (R22)                              */
+    int32_t layout;          /* LVSA_LAYOUT_*                                                   */
     int64_t N;               /* T*P + n_text                                                    */
     int64_t nnz;             /* kept (q tile, kv tile) pairs                                    */
     int64_t n_partial;       /* of which PARTIAL                                                */
@@ -99,8 +111,12 @@ typedef struct lvsa_index_info {
  * round trip); the counters (nnz, ...) are read back lazily by lvsa_index_info /
  * lvsa_index_copy_host, which do synchronise.  Use the index on the stream it was built on (or
  * order other streams after it).  Returns NULL on error (lvsa_last_error()).
- * The handle is owned by the library; free it with lvsa_index_destroy.  It is immutable and
- * may be used by any number of lvsa_attn_fwd calls.
+ * The handle is owned by the library; free it with lvsa_index_destroy.  Its contents never change
+ * and it may be used by any number of lvsa_attn_fwd calls, but a handle is NOT thread-safe: the
+ * library records on it which stream used it last (to free its stream-ordered memory behind that
+ * work), so calls that share one handle must be serialised by the caller.  Different handles may
+ * be used from different threads.  The index belongs to the device that was current when it was
+ * built; every later call with it must be made with that device current (else LVSA_EINVAL).
  */
 lvsa_index_t *lvsa_build_block_index(int T, int P, int H, int d, int window, int anchors,
                                      int step, int layer);
@@ -112,11 +128,12 @@ lvsa_status_t lvsa_build_block_index_ex(const lvsa_params_t *params, void *strea
 /*
  * lvsa_attn_fwd — step a6/a7: Eq. 2 over the kept tiles, exactly (element-level masking on
  * PARTIAL tiles).
- *   q, k, v : DEVICE pointers, [B, N, H, d] contiguous (d fastest), bf16 (or fp32 when the index
- *             was built with LVSA_DTYPE_FP32); 16-byte aligned.  Read-only.
- *   out     : DEVICE pointer, same shape and dtype as q.  Every element is written.
- *   lse     : DEVICE pointer, fp32 [B, H, N], lse = ln sum_{kept} exp(q.k/sqrt d) (natural log),
- *             or NULL.
+ *   q, k, v : DEVICE pointers, contiguous [B, N, H, d] (or [B, H, N, d] when the index was built
+ *             with LVSA_LAYOUT_HND), d fastest, bf16 (or fp32 when the index was built with
+ *             LVSA_DTYPE_FP32); 16-byte aligned.  Read-only.
+ *   out     : DEVICE pointer, same shape, layout and dtype as q.  Every element is written.
+ *   lse     : DEVICE pointer, fp32 [B, H, N], 4-byte aligned, lse = ln sum_{kept} exp(q.k/sqrt d)
+ *             (natural log), or NULL.
  *   stream  : cudaStream_t of the caller (NULL = default stream).
  * The call only enqueues work on `stream` and returns; it never synchronises and allocates
  * nothing.  Caller owns all five buffers; the library keeps no reference after the kernels ran.
@@ -131,11 +148,13 @@ lvsa_status_t lvsa_attn_fwd(const void *q, const void *k, const void *v,
  * a device workspace owned by the library (one per process, allocated on first use, grown on
  * demand, shared by all indices; freed by lvsa_workspace_release), runs lvsa_attn_fwd on
  * `stream`, copies out (and lse if not NULL) back, and synchronises `stream` before returning.
- * With the CTA-pair kernel (bf16, d = 128) the call is pipelined over groups of heads (by default one
- * head per group, at most 16 groups; LVSA_HOST_GROUPS overrides): the host-to-device copy of the next group and the
- * device-to-host copy of the previous one run on two internal streams while the kernel of the
- * current group runs on `stream`.  Results are identical to the unpipelined call.
- * Calls through the workspace are serialised by a mutex.
+ * With the CTA-pair kernel (bf16, d = 128) the call is pipelined over groups of heads (by default
+ * one head per group, at most 16 groups; lvsa_params_t.host_groups overrides): the host-to-device
+ * copy of the next group and the device-to-host copy of the previous one run on two internal
+ * streams while the kernel of the current group runs on `stream`.  Results are identical to the
+ * unpipelined call.  Calls through the workspace are serialised by a mutex.  If a CUDA call fails
+ * part-way, the call waits for everything it enqueued before it returns the error, so no copy is
+ * still reading or writing the caller's host buffers afterwards.
  */
 lvsa_status_t lvsa_attn_fwd_host(const void *q_host, const void *k_host, const void *v_host,
                                  lvsa_index_t *index, void *out_host, float *lse_host,
@@ -174,8 +193,9 @@ void lvsa_index_destroy(lvsa_index_t *index);
 lvsa_status_t lvsa_index_info(const lvsa_index_t *index, lvsa_index_info_t *info);
 
 /* Copies the index to HOST arrays sized from lvsa_index_info (any pointer may be NULL):
- * indptr[nq+1], indices[nnz], flags[nnz], w_lo[T], w_hi[T], a_bits[T*words] (bit x of row t set
- * iff x in A(t), little-endian words).  Synchronises. */
+ * indptr[nq+1], indices[nnz], flags[nnz], w_lo[T], w_hi[T], a_bits[T'*words] with T' = T +
+ * (n_text > 0 ? 1 : 0) rows (bit x of row t set iff x in A(t), little-endian words; row T is the
+ * text pseudo-frame, R23).  Synchronises. */
 lvsa_status_t lvsa_index_copy_host(const lvsa_index_t *index, int32_t *indptr, int32_t *indices,
                                    uint8_t *flags, int32_t *w_lo, int32_t *w_hi,
                                    uint32_t *a_bits);

@@ -20,7 +20,8 @@ ALL_TILES = -1
 TILE_FULL, TILE_PARTIAL = 0, 1
 TIE_LO, TIE_HI = 0, 1
 DTYPE_BF16, DTYPE_FP32 = 0, 1
-KERNEL_AUTO, KERNEL_SIMT, KERNEL_TCGEN05 = 0, 1, 2
+KERNEL_AUTO, KERNEL_SIMT, KERNEL_TCGEN05, KERNEL_TCGEN05_V0 = 0, 1, 2, 3
+LAYOUT_NHD, LAYOUT_HND = 0, 1
 OK, EINVAL, EUNSUPPORTED, ECUDA, ENOMEM = 0, 1, 2, 3, 4
 
 
@@ -35,14 +36,16 @@ class Params(C.Structure):
                 ("T", "P", "H", "d", "B", "window", "anchors", "step", "layer", "tile_q", "tile_k",
                  "tie_break", "dtype", "kernel")] + [("softmax_scale", C.c_float),
                                                      ("initial_anchors", C.c_int32),
-                                                     ("n_text", C.c_int32)]
+                                                     ("n_text", C.c_int32),
+                                                     ("layout", C.c_int32),
+                                                     ("host_groups", C.c_int32)]
 
 
 class IndexInfo(C.Structure):
     _fields_ = [(n, C.c_int32) for n in
                 ("T", "P", "H", "d", "B", "window", "anchors", "step", "layer", "tile_q", "tile_k",
                  "nq", "nk", "T_per", "phase", "n_global", "words", "dtype", "kernel", "n_text",
-                 "initial_anchors")] + \
+                 "initial_anchors", "layout")] + \
                [(n, C.c_int64) for n in ("N", "nnz", "n_partial", "n_items", "n_item_tiles")]
 
 
@@ -192,7 +195,8 @@ def _dev_ptr(t) -> C.c_void_p:
 
 
 def lvsa_attn_fwd(q, k, v, index: BlockIndex, out, lse=None, stream: int | None = None):
-    """q, k, v, out: CUDA tensors [B, N, H, d]; lse: CUDA fp32 [B, H, N] or None.  Enqueues on
+    """q, k, v, out: CUDA tensors [B, N, H, d] (or [B, H, N, d] for an index built with
+    layout=LAYOUT_HND); lse: CUDA fp32 [B, H, N] or None.  Enqueues on
     `stream` (default: torch's current stream) and returns without synchronising."""
     if stream is None:
         import torch

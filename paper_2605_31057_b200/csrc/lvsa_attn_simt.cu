@@ -29,7 +29,8 @@ lvsa_attn_simt_kernel(const T *__restrict__ q, const T *__restrict__ k, const T 
                       T *__restrict__ out, float *__restrict__ lse,
                       const int32_t *__restrict__ indptr, const int32_t *__restrict__ indices,
                       const uint8_t *__restrict__ flags, const uint32_t *__restrict__ a_bits,
-                      int words, long long N, int P, int Tf, int H, float scale) {
+                      int words, long long N, int P, int Tf, int H, long long sn, long long sh, long long sb,
+                      float scale) {
     constexpr int R = BT / SIMT_WARPS;  // rows per warp
     constexpr int CH = D / 32;          // output channels per lane
     constexpr int KS = D + 1;           // padded K row (lane c reads row c: conflict-free)
@@ -40,10 +41,11 @@ lvsa_attn_simt_kernel(const T *__restrict__ q, const T *__restrict__ k, const T 
     const int i = blockIdx.x, h = blockIdx.y, b = blockIdx.z;
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const long long row0 = (long long)i * BT;
-    const size_t tok_stride = (size_t)H * D;
-    const T *qb = q + (size_t)b * N * tok_stride + (size_t)h * D;
-    const T *kb = k + (size_t)b * N * tok_stride + (size_t)h * D;
-    const T *vb = v + (size_t)b * N * tok_stride + (size_t)h * D;
+    const size_t tok_stride = (size_t)sn;                                  // token / head / batch strides:
+    const size_t base_off = (size_t)b * (size_t)sb + (size_t)h * (size_t)sh;  // lvsa_params_t.layout
+    const T *qb = q + base_off;
+    const T *kb = k + base_off;
+    const T *vb = v + base_off;
 
     for (int e = tid; e < BT * D; e += blockDim.x) {
         const int r = e / D, c = e % D;
@@ -117,7 +119,7 @@ lvsa_attn_simt_kernel(const T *__restrict__ q, const T *__restrict__ k, const T 
         }
     }
 
-    T *ob = out + (size_t)b * N * tok_stride + (size_t)h * D;
+    T *ob = out + base_off;
 #pragma unroll
     for (int r = 0; r < R; ++r) {
         const int rl = wid + r * SIMT_WARPS;
@@ -139,10 +141,11 @@ lvsa_status_t launch(const lvsa_index *ix, const void *q, const void *k, const v
     auto kern = lvsa_attn_simt_kernel<D, BT, T>;
     LVSA_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const float scale = ix->p.softmax_scale;
+    const lvsa_strides sd = lvsa_layout_strides(ix);
     dim3 grid(ix->nq, ix->p.H, ix->p.B);
     kern<<<grid, SIMT_WARPS * 32, smem, stream>>>(
         (const T *)q, (const T *)k, (const T *)v, (T *)out, lse, ix->d_indptr, ix->d_indices,
-        ix->d_flags, ix->d_abits, ix->words, (long long)ix->N, ix->p.P, ix->Tf, ix->p.H, scale);
+        ix->d_flags, ix->d_abits, ix->words, (long long)ix->N, ix->p.P, ix->Tf, ix->p.H, sd.n, sd.h, sd.b, scale);
     LVSA_CUDA_TRY(cudaGetLastError());
     return LVSA_OK;
 }

@@ -12,8 +12,6 @@
 #include <cuda.h>
 #include <cuda_bf16.h>
 
-#include <stdlib.h>
-
 #include "lvsa_internal.h"
 #include "sm100_ptx.cuh"
 
@@ -53,7 +51,7 @@ lvsa_attn_sm100_v0_kernel(const __grid_constant__ CUtensorMap tmap_q,
                           __nv_bfloat16 *__restrict__ out, float *__restrict__ lse,
                           const int32_t *__restrict__ item_ptr, const int32_t *__restrict__ item_tiles,
                           const uint32_t *__restrict__ a_bits, int words, long long N, int P, int T,
-                          int H, float scale_log2, float *__restrict__ dbg) {
+                          int H, long long sn, long long sh, long long sb, float scale_log2) {
     using C = Cfg<D, BT>;
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -154,9 +152,6 @@ lvsa_attn_sm100_v0_kernel(const __grid_constant__ CUtensorMap tmap_q,
                 for (int x = 0; x < 32; ++x) s[c * 32 + x] = __uint_as_float(r[x]);
             }
             tmem_wait_ld();
-            if (dbg != nullptr && item == 0 && h == 0 && b == 0 && e == e0) {
-                for (int c = 0; c < BT; ++c) dbg[(size_t)(wg * 128 + rw) * BT + c] = s[c];
-            }
             if (st_row != LVSA_ST_FULL) {
                 uint32_t cm[BT / 32];
 #pragma unroll
@@ -242,7 +237,7 @@ lvsa_attn_sm100_v0_kernel(const __grid_constant__ CUtensorMap tmap_q,
     if (started) {
         const bool row_ok = my_row < N;
         const float inv = 1.f / l_run;
-        __nv_bfloat16 *orow = out + (((size_t)b * N + (row_ok ? my_row : 0)) * H + h) * D;
+        __nv_bfloat16 *orow = out + (size_t)b * sb + (size_t)(row_ok ? my_row : 0) * sn + (size_t)h * sh;
 #pragma unroll
         for (int c = 0; c < D / 32; ++c) {
             uint32_t r[32];
@@ -287,13 +282,18 @@ PFN_encodeTiled get_encode() {
 
 }  // namespace
 
-// [B, N, H, d] bf16, d fastest.  Tensor-map dims (fastest first): d, H, N, B.  Box: 64 x 1 x rows x 1
-// with SWIZZLE_128B, i.e. smem tile [rows][128 B]; rows >= N are zero-filled.
-lvsa_status_t lvsa_make_tmap_bf16(CUtensorMap *m, const void *base, long long N, int H, int d, int B, int box_rows) {
+// bf16 tensor with axes (d, H, N, B), d contiguous; element strides of the token / head / batch axes
+// from lvsa_layout_strides (NHD or HND).  Tensor-map dims (fastest first): d, H, N, B whatever the
+// memory order (TMA strides need not be sorted).  Box: 64 x 1 x rows x 1 with SWIZZLE_128B, i.e.
+// smem tile [rows][128 B]; rows >= N are zero-filled.
+lvsa_status_t lvsa_make_tmap_bf16(CUtensorMap *m, const void *base, const lvsa_index *ix, int box_rows) {
+    const long long N = ix->N;
+    const int H = ix->p.H, d = ix->p.d, B = ix->p.B;
+    const lvsa_strides sd = lvsa_layout_strides(ix);
     PFN_encodeTiled enc = get_encode();
     if (enc == nullptr) { lvsa_set_error("cuTensorMapEncodeTiled entry point not found"); return LVSA_ECUDA; }
     cuuint64_t dims[4] = {(cuuint64_t)d, (cuuint64_t)H, (cuuint64_t)N, (cuuint64_t)B};
-    cuuint64_t strides[3] = {(cuuint64_t)d * 2, (cuuint64_t)H * d * 2, (cuuint64_t)N * H * d * 2};
+    cuuint64_t strides[3] = {(cuuint64_t)sd.h * 2, (cuuint64_t)sd.n * 2, (cuuint64_t)sd.b * 2};
     cuuint32_t box[4] = {64, 1, (cuuint32_t)box_rows, 1};
     cuuint32_t estr[4] = {1, 1, 1, 1};
     CUresult r = enc(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, const_cast<void *>(base), dims, strides, box, estr,
@@ -308,38 +308,40 @@ lvsa_status_t lvsa_make_tmap_bf16(CUtensorMap *m, const void *base, long long N,
 
 namespace {
 
-float *g_dbg = nullptr;
-
 template <int D, int BT>
 lvsa_status_t launch_v0(const lvsa_index *ix, const void *q, const void *k, const void *v, void *out,
                         float *lse, cudaStream_t stream) {
     using C = Cfg<D, BT>;
     CUtensorMap mq, mk, mv;
     lvsa_status_t st;
-    if ((st = lvsa_make_tmap_bf16(&mq, q, ix->N, ix->p.H, D, ix->p.B, 128)) != LVSA_OK) return st;
-    if ((st = lvsa_make_tmap_bf16(&mk, k, ix->N, ix->p.H, D, ix->p.B, BT)) != LVSA_OK) return st;
-    if ((st = lvsa_make_tmap_bf16(&mv, v, ix->N, ix->p.H, D, ix->p.B, BT)) != LVSA_OK) return st;
+    if ((st = lvsa_make_tmap_bf16(&mq, q, ix, 128)) != LVSA_OK) return st;
+    if ((st = lvsa_make_tmap_bf16(&mk, k, ix, BT)) != LVSA_OK) return st;
+    if ((st = lvsa_make_tmap_bf16(&mv, v, ix, BT)) != LVSA_OK) return st;
     auto kern = lvsa_attn_sm100_v0_kernel<D, BT>;
-    LVSA_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
+    // the attribute is per device: set once per (instantiation, device)
+    static bool ready[LVSA_MAX_DEVICES] = {};
+    if (!ready[ix->device]) {
+        LVSA_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
+        ready[ix->device] = true;
+    }
     const float scale_log2 = ix->p.softmax_scale * 1.4426950408889634f;
+    const lvsa_strides sd = lvsa_layout_strides(ix);
     dim3 grid((unsigned)ix->n_items, ix->p.H, ix->p.B);
     kern<<<grid, C::NWG * 128, C::SMEM_BYTES, stream>>>(
         mq, mk, mv, (__nv_bfloat16 *)out, lse, ix->d_item_ptr, ix->d_item_tiles, ix->d_abits, ix->words,
-        (long long)ix->N, ix->p.P, ix->Tf, ix->p.H, scale_log2, g_dbg);
+        (long long)ix->N, ix->p.P, ix->Tf, ix->p.H, sd.n, sd.h, sd.b, scale_log2);
     LVSA_CUDA_TRY(cudaGetLastError());
     return LVSA_OK;
 }
 
 }  // namespace
 
-extern "C" void lvsa_debug_set_dump(float *dev_ptr) { g_dbg = dev_ptr; }
-
 int lvsa_attn_sm100_supported(const lvsa_index *ix) {
     // compute-capability major per device, queried once (cudaGetDeviceProperties costs milliseconds
     // and this runs in every index build)
-    static int cc_major[64] = {};
+    static int cc_major[LVSA_MAX_DEVICES] = {};
     const int dev = ix->device;
-    if (dev < 0 || dev >= 64) return 0;
+    if (dev < 0 || dev >= LVSA_MAX_DEVICES) return 0;
     if (cc_major[dev] == 0) {
         int v = 0;
         if (cudaDeviceGetAttribute(&v, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess) return 0;
@@ -349,15 +351,9 @@ int lvsa_attn_sm100_supported(const lvsa_index *ix) {
     return (ix->p.d == 128 && ix->p.tile_q == 128) || (ix->p.d == 64 && ix->p.tile_q == 64);
 }
 
-static bool pair_disabled() {
-    // LVSA_PAIR=0 selects the one-CTA warp-specialised kernel (A/B timing; same results)
-    static const bool no_pair = getenv("LVSA_PAIR") != nullptr && getenv("LVSA_PAIR")[0] == '0';
-    return no_pair;
-}
-
+// d = 128: the CTA-pair kernel unless the index asks for the one-CTA-per-item kernel
 int lvsa_attn_uses_pair_kernel(const lvsa_index *ix) {
-    static const bool force_v0 = getenv("LVSA_SM100_V0") != nullptr && getenv("LVSA_SM100_V0")[0] == '1';
-    return ix->p.d == 128 && !force_v0 && g_dbg == nullptr && !pair_disabled();
+    return ix->p.d == 128 && ix->p.kernel != LVSA_KERNEL_TCGEN05_V0;
 }
 
 lvsa_status_t lvsa_attn_sm100_launch(const lvsa_index *ix, const void *q, const void *k,
@@ -367,11 +363,8 @@ lvsa_status_t lvsa_attn_sm100_launch(const lvsa_index *ix, const void *q, const 
         return LVSA_EUNSUPPORTED;
     }
     if (ix->p.d == 128) {
-        // LVSA_SM100_V0=1 selects the bring-up kernel (debugging aid; same results)
-        static const bool force_v0 = getenv("LVSA_SM100_V0") != nullptr && getenv("LVSA_SM100_V0")[0] == '1';
-        if (force_v0 || g_dbg != nullptr) return launch_v0<128, 128>(ix, q, k, v, out, lse, stream);
-        if (!pair_disabled()) return lvsa_attn_sm100_pair_launch(ix, q, k, v, out, lse, stream);
-        return lvsa_attn_sm100_ws_launch(ix, q, k, v, out, lse, stream);
+        if (lvsa_attn_uses_pair_kernel(ix)) return lvsa_attn_sm100_pair_launch(ix, q, k, v, out, lse, stream);
+        return launch_v0<128, 128>(ix, q, k, v, out, lse, stream);
     }
     return launch_v0<64, 64>(ix, q, k, v, out, lse, stream);
 }

@@ -81,7 +81,8 @@ lvsa_attn_sm100_pair_kernel(const __grid_constant__ CUtensorMap tmap_q,
                             __nv_bfloat16 *__restrict__ out, float *__restrict__ lse,
                             const int32_t *__restrict__ item_ptr, const int32_t *__restrict__ item_tiles,
                             const uint32_t *__restrict__ a_bits, int words, long long N, int P, int T,
-                            int H, int h0, int hc, int n_items, long long n_work, float scale_log2) {
+                            int H, int h0, int hc, int n_items, long long n_work, long long sn, long long sh,
+                            long long sb, float scale_log2) {
     using SM = SmemP<NS>;
     extern __shared__ __align__(1024) uint8_t smem_raw[];
     const uint32_t base = smem_u32(smem_raw);
@@ -304,7 +305,7 @@ lvsa_attn_sm100_pair_kernel(const __grid_constant__ CUtensorMap tmap_q,
                 pair_sync();   // m_ref and the exchange slots are free again for the next item
                 const bool row_ok = my_row < N;
                 const float inv = 1.f / l_tot;
-                __nv_bfloat16 *orow = out + (((size_t)b * N + (row_ok ? my_row : 0)) * H + h) * D + w * CH;
+                __nv_bfloat16 *orow = out + (size_t)b * sb + (size_t)(row_ok ? my_row : 0) * sn + (size_t)h * sh + w * CH;
 #pragma unroll
                 for (int c = 0; c < 2; ++c) {
                     uint32_t r[32];
@@ -469,18 +470,20 @@ lvsa_attn_sm100_pair_kernel(const __grid_constant__ CUtensorMap tmap_q,
 }  // namespace
 
 // host side -------------------------------------------------------------------------------
-lvsa_status_t lvsa_make_tmap_bf16(CUtensorMap *m, const void *base, long long N, int H, int d, int B,
-                                  int box_rows);
+lvsa_status_t lvsa_make_tmap_bf16(CUtensorMap *m, const void *base, const lvsa_index *ix, int box_rows);
 
-static int g_pair_n_sm = 0;
+// One-time setup per DEVICE (the shared-memory attribute and the SM count belong to a device, not
+// to the process); `device` must be the current device.
+static int g_pair_n_sm[LVSA_MAX_DEVICES] = {};
 lvsa_status_t lvsa_attn_sm100_pair_prepare(int device) {
-    if (g_pair_n_sm != 0) return LVSA_OK;
+    if (device < 0 || device >= LVSA_MAX_DEVICES) { lvsa_set_error("device ordinal out of range"); return LVSA_EUNSUPPORTED; }
+    if (g_pair_n_sm[device] != 0) return LVSA_OK;
     using SM = SmemP<LVSA_PAIR_STAGES>;
     LVSA_CUDA_TRY(cudaFuncSetAttribute(lvsa_attn_sm100_pair_kernel<LVSA_PAIR_STAGES>,
                                        cudaFuncAttributeMaxDynamicSharedMemorySize, SM::BYTES));
     int n = 0;
     LVSA_CUDA_TRY(cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, device));
-    g_pair_n_sm = n;
+    g_pair_n_sm[device] = n;
     return LVSA_OK;
 }
 
@@ -492,17 +495,18 @@ lvsa_status_t lvsa_attn_sm100_pair_launch_heads(const lvsa_index *ix, const void
     using SM = SmemP<NS>;
     CUtensorMap mq, mk, mv;
     lvsa_status_t st;
-    if ((st = lvsa_make_tmap_bf16(&mq, q, ix->N, ix->p.H, D, ix->p.B, 128)) != LVSA_OK) return st;
-    if ((st = lvsa_make_tmap_bf16(&mk, k, ix->N, ix->p.H, D, ix->p.B, 64)) != LVSA_OK) return st;
-    if ((st = lvsa_make_tmap_bf16(&mv, v, ix->N, ix->p.H, D, ix->p.B, BT)) != LVSA_OK) return st;
+    if ((st = lvsa_make_tmap_bf16(&mq, q, ix, 128)) != LVSA_OK) return st;
+    if ((st = lvsa_make_tmap_bf16(&mk, k, ix, 64)) != LVSA_OK) return st;
+    if ((st = lvsa_make_tmap_bf16(&mv, v, ix, BT)) != LVSA_OK) return st;
     if ((st = lvsa_attn_sm100_pair_prepare(ix->device)) != LVSA_OK) return st;
     const long long n_work = (long long)ix->n_items * hc * ix->p.B;
-    long long n_pairs = g_pair_n_sm / 2;
+    long long n_pairs = g_pair_n_sm[ix->device] / 2;
+    const lvsa_strides sd = lvsa_layout_strides(ix);
     if (n_work < n_pairs) n_pairs = n_work;
     const float scale_log2 = ix->p.softmax_scale * 1.4426950408889634f;
     lvsa_attn_sm100_pair_kernel<NS><<<(unsigned)(2 * n_pairs), NTHREADS, SM::BYTES, stream>>>(
         mq, mk, mv, (__nv_bfloat16 *)out, lse, ix->d_item_ptr, ix->d_item_tiles, ix->d_abits, ix->words,
-        (long long)ix->N, ix->p.P, ix->Tf, ix->p.H, h0, hc, (int)ix->n_items, n_work, scale_log2);
+        (long long)ix->N, ix->p.P, ix->Tf, ix->p.H, h0, hc, (int)ix->n_items, n_work, sd.n, sd.h, sd.b, scale_log2);
     LVSA_CUDA_TRY(cudaGetLastError());
     return LVSA_OK;
 }

@@ -17,17 +17,31 @@ lvsa_status_t lvsa_cuda_fail(cudaError_t e, const char *what) {
     return LVSA_ECUDA;
 }
 
-// staging buffers of lvsa_attn_fwd_host (process-wide, one device at a time)
-static struct { void *ptr = nullptr; size_t cap = 0; int device = -1; } g_ws;
+// staging buffers of lvsa_attn_fwd_host: one workspace per DEVICE, process lifetime (or until
+// lvsa_workspace_release), guarded by one mutex
+struct HostWorkspace { void *ptr = nullptr; size_t cap = 0; };
+static HostWorkspace g_ws[LVSA_MAX_DEVICES];
 static std::mutex g_ws_mutex;
 
-// streams and events of the pipelined host entry point (created on first use, process lifetime)
+// streams and events of the pipelined host entry point (per device, created on first use)
 struct HostPipe {
     static constexpr int MAXG = 16;
     cudaStream_t s_in = nullptr, s_out = nullptr;
     cudaEvent_t ev_in[MAXG] = {}, ev_c[MAXG] = {}, ev_edge = nullptr;
 };
-static HostPipe g_host;
+static HostPipe g_host[LVSA_MAX_DEVICES];
+
+// the index belongs to one device; every call that uses it must run with that device current
+static lvsa_status_t check_device(const lvsa_index *ix) {
+    int dev = -1;
+    LVSA_CUDA_TRY(cudaGetDevice(&dev));
+    if (dev != ix->device) {
+        lvsa_set_error("the index was built on device " + std::to_string(ix->device) + " but device " +
+                       std::to_string(dev) + " is current");
+        return LVSA_EINVAL;
+    }
+    return LVSA_OK;
+}
 
 // records that `stream` used the index (its arena is stream-ordered memory)
 static bool index_touch_stream(const lvsa_index *index, cudaStream_t stream) {
@@ -43,16 +57,13 @@ static size_t elem_size(const lvsa_index *ix) { return ix->p.dtype == LVSA_DTYPE
 
 static int use_tcgen05(const lvsa_index *ix) {
     if (ix->p.kernel == LVSA_KERNEL_SIMT) return 0;
-    if (ix->p.kernel == LVSA_KERNEL_TCGEN05) return 1;
+    if (ix->p.kernel == LVSA_KERNEL_TCGEN05 || ix->p.kernel == LVSA_KERNEL_TCGEN05_V0) return 1;
     return ix->p.dtype == LVSA_DTYPE_BF16;
 }
 
 lvsa_status_t lvsa_attn_prepare(const lvsa_index *ix) {
-    if (use_tcgen05(ix) && ix->p.d == 128) {
-        lvsa_status_t st = lvsa_attn_sm100_pair_prepare(ix->device);
-        return st != LVSA_OK ? st : lvsa_attn_sm100_ws_prepare(ix->device);
-    }
-    return LVSA_OK;   // the other kernels set their attributes at launch
+    if (use_tcgen05(ix) && lvsa_attn_uses_pair_kernel(ix)) return lvsa_attn_sm100_pair_prepare(ix->device);
+    return LVSA_OK;   // the other kernels set their attributes at their first launch
 }
 
 extern "C" {
@@ -60,7 +71,7 @@ extern "C" {
 const char *lvsa_last_error(void) { return g_last_error.c_str(); }
 
 const char *lvsa_version(void) {
-    return "liblvsa 0.1 (sm_100a; kernels: index-builder, attn-simt-fp32, attn-tcgen05-bf16 (CTA-pair cta_group::2, one-CTA warp-specialised, v0))";
+    return "liblvsa 0.2 (sm_100a; kernels: index-builder, attn-simt-fp32, attn-tcgen05-bf16 (CTA-pair cta_group::2; one-CTA v0))";
 }
 
 lvsa_status_t lvsa_build_block_index_ex(const lvsa_params_t *params, void *stream, lvsa_index_t **out) {
@@ -79,7 +90,9 @@ lvsa_status_t lvsa_build_block_index_ex(const lvsa_params_t *params, void *strea
     if (p.n_text < 0) { lvsa_set_error("n_text must be >= 0"); return LVSA_EINVAL; }
     if (p.tie_break != LVSA_TIE_LO && p.tie_break != LVSA_TIE_HI) { lvsa_set_error("bad tie_break"); return LVSA_EINVAL; }
     if (p.dtype != LVSA_DTYPE_BF16 && p.dtype != LVSA_DTYPE_FP32) { lvsa_set_error("bad dtype"); return LVSA_EINVAL; }
-    if (p.kernel < LVSA_KERNEL_AUTO || p.kernel > LVSA_KERNEL_TCGEN05) { lvsa_set_error("bad kernel"); return LVSA_EINVAL; }
+    if (p.kernel < LVSA_KERNEL_AUTO || p.kernel > LVSA_KERNEL_TCGEN05_V0) { lvsa_set_error("bad kernel"); return LVSA_EINVAL; }
+    if (p.layout != LVSA_LAYOUT_NHD && p.layout != LVSA_LAYOUT_HND) { lvsa_set_error("bad layout"); return LVSA_EINVAL; }
+    if (p.host_groups < 0) { lvsa_set_error("host_groups must be >= 0"); return LVSA_EINVAL; }
     if (p.T > 4096) { lvsa_set_error("T > 4096 frames is not supported"); return LVSA_EUNSUPPORTED; }
     if (p.d != 64 && p.d != 128) { lvsa_set_error("head dim must be 64 or 128"); return LVSA_EUNSUPPORTED; }
     if (p.tile_q == 0) p.tile_q = p.d;
@@ -88,7 +101,7 @@ lvsa_status_t lvsa_build_block_index_ex(const lvsa_params_t *params, void *strea
         lvsa_set_error("tiles must be 128x128 for d = 128 and 64x64 for d = 64");
         return LVSA_EUNSUPPORTED;
     }
-    if (p.dtype == LVSA_DTYPE_FP32 && p.kernel == LVSA_KERNEL_TCGEN05) {
+    if (p.dtype == LVSA_DTYPE_FP32 && (p.kernel == LVSA_KERNEL_TCGEN05 || p.kernel == LVSA_KERNEL_TCGEN05_V0)) {
         lvsa_set_error("the tcgen05 kernel takes bf16 only");
         return LVSA_EUNSUPPORTED;
     }
@@ -110,6 +123,7 @@ lvsa_status_t lvsa_build_block_index_ex(const lvsa_params_t *params, void *strea
     }
     cudaError_t e = cudaGetDevice(&ix->device);
     if (e != cudaSuccess) { lvsa_index_destroy(ix); return lvsa_cuda_fail(e, "cudaGetDevice (no usable CUDA device; there is no CPU fallback)"); }
+    if (ix->device < 0 || ix->device >= LVSA_MAX_DEVICES) { lvsa_index_destroy(ix); lvsa_set_error("device ordinal out of range"); return LVSA_EUNSUPPORTED; }
     lvsa_status_t st = lvsa_index_build_device(ix, (cudaStream_t)stream);
     if (st != LVSA_OK) { lvsa_index_destroy(ix); return st; }
     if (use_tcgen05(ix) && !lvsa_attn_sm100_supported(ix)) {
@@ -142,9 +156,76 @@ lvsa_status_t lvsa_attn_fwd(const void *q, const void *k, const void *v, const l
         lvsa_set_error("q, k, v, out must be 16-byte aligned");
         return LVSA_EINVAL;
     }
+    if ((uintptr_t)lse & 3u) { lvsa_set_error("lse must be 4-byte aligned"); return LVSA_EINVAL; }
+    lvsa_status_t dst = check_device(index);
+    if (dst != LVSA_OK) return dst;
     index_touch_stream(index, (cudaStream_t)stream);   // the arena is stream-ordered memory
     if (use_tcgen05(index)) return lvsa_attn_sm100_launch(index, q, k, v, out, lse, (cudaStream_t)stream);
     return lvsa_attn_simt_launch(index, q, k, v, out, lse, (cudaStream_t)stream);
+}
+
+// The pipelined body of lvsa_attn_fwd_host: everything it enqueues goes to `stream`, hp.s_in and
+// hp.s_out; the caller synchronises all three whatever this returns.
+static lvsa_status_t host_pipeline(lvsa_index *ix, HostPipe &hp, int G, const void *qh, const void *kh, const void *vh,
+                                   void *oh, float *lseh, void *s_q, void *s_k, void *s_v, void *s_o,
+                                   float *s_lse, cudaStream_t stream) {
+    const int H = ix->p.H;
+    const size_t es = elem_size(ix);
+    const int per = (H + G - 1) / G;
+    // One head group = a strided 2-D block of the tensor: NHD [B*N rows][H*d] -> hc*d wide columns of
+    // every token row; HND [B rows][H*N*d] -> hc*N*d contiguous elements of every batch.
+    const bool hnd = ix->p.layout == LVSA_LAYOUT_HND;
+    const size_t pitch = hnd ? (size_t)H * ix->N * ix->p.d * es : (size_t)H * ix->p.d * es;
+    const size_t rows = hnd ? (size_t)ix->p.B : (size_t)ix->p.B * ix->N;
+    const size_t per_head = hnd ? (size_t)ix->N * ix->p.d * es : (size_t)ix->p.d * es;
+    // copies start after whatever the caller already enqueued on `stream`
+    LVSA_CUDA_TRY(cudaEventRecord(hp.ev_edge, stream));
+    LVSA_CUDA_TRY(cudaStreamWaitEvent(hp.s_in, hp.ev_edge, 0));
+    LVSA_CUDA_TRY(cudaStreamWaitEvent(hp.s_out, hp.ev_edge, 0));
+    int ng = 0;
+    for (int h0 = 0; h0 < H; h0 += per, ++ng) {
+        const int hc = h0 + per <= H ? per : H - h0;
+        const size_t off = (size_t)h0 * per_head, width = (size_t)hc * per_head;
+        const void *src[3] = {qh, kh, vh};
+        void *dst[3] = {s_q, s_k, s_v};
+        for (int t = 0; t < 3; ++t)
+            LVSA_CUDA_TRY(cudaMemcpy2DAsync((uint8_t *)dst[t] + off, pitch, (const uint8_t *)src[t] + off, pitch, width,
+                                            rows, cudaMemcpyHostToDevice, hp.s_in));
+        LVSA_CUDA_TRY(cudaEventRecord(hp.ev_in[ng], hp.s_in));
+    }
+    ng = 0;
+    for (int h0 = 0; h0 < H; h0 += per, ++ng) {
+        const int hc = h0 + per <= H ? per : H - h0;
+        const size_t off = (size_t)h0 * per_head, width = (size_t)hc * per_head;
+        LVSA_CUDA_TRY(cudaStreamWaitEvent(stream, hp.ev_in[ng], 0));
+        lvsa_status_t st = lvsa_attn_sm100_pair_launch_heads(ix, s_q, s_k, s_v, s_o, s_lse, h0, hc, stream);
+        if (st != LVSA_OK) return st;
+        LVSA_CUDA_TRY(cudaEventRecord(hp.ev_c[ng], stream));
+        LVSA_CUDA_TRY(cudaStreamWaitEvent(hp.s_out, hp.ev_c[ng], 0));
+        LVSA_CUDA_TRY(cudaMemcpy2DAsync((uint8_t *)oh + off, pitch, (const uint8_t *)s_o + off, pitch, width, rows,
+                                        cudaMemcpyDeviceToHost, hp.s_out));
+        if (lseh != nullptr)   // lse is [B, H, N]: heads h0.. of every batch are contiguous runs of hc * N floats
+            LVSA_CUDA_TRY(cudaMemcpy2DAsync(lseh + (size_t)h0 * ix->N, sizeof(float) * (size_t)H * ix->N,
+                                            s_lse + (size_t)h0 * ix->N, sizeof(float) * (size_t)H * ix->N,
+                                            sizeof(float) * (size_t)hc * ix->N, (size_t)ix->p.B,
+                                            cudaMemcpyDeviceToHost, hp.s_out));
+    }
+    LVSA_CUDA_TRY(cudaEventRecord(hp.ev_edge, hp.s_out));
+    LVSA_CUDA_TRY(cudaStreamWaitEvent(stream, hp.ev_edge, 0));
+    return LVSA_OK;
+}
+
+static lvsa_status_t host_plain(lvsa_index *ix, size_t bytes, size_t lbytes, const void *qh, const void *kh,
+                                const void *vh, void *oh, float *lseh, void *s_q, void *s_k, void *s_v, void *s_o,
+                                float *s_lse, cudaStream_t stream) {
+    LVSA_CUDA_TRY(cudaMemcpyAsync(s_q, qh, bytes, cudaMemcpyHostToDevice, stream));
+    LVSA_CUDA_TRY(cudaMemcpyAsync(s_k, kh, bytes, cudaMemcpyHostToDevice, stream));
+    LVSA_CUDA_TRY(cudaMemcpyAsync(s_v, vh, bytes, cudaMemcpyHostToDevice, stream));
+    lvsa_status_t st = lvsa_attn_fwd(s_q, s_k, s_v, ix, s_o, s_lse, stream);
+    if (st != LVSA_OK) return st;
+    LVSA_CUDA_TRY(cudaMemcpyAsync(oh, s_o, bytes, cudaMemcpyDeviceToHost, stream));
+    if (lseh != nullptr) LVSA_CUDA_TRY(cudaMemcpyAsync(lseh, s_lse, lbytes, cudaMemcpyDeviceToHost, stream));
+    return LVSA_OK;
 }
 
 lvsa_status_t lvsa_attn_fwd_host(const void *qh, const void *kh, const void *vh, lvsa_index_t *ix,
@@ -153,96 +234,73 @@ lvsa_status_t lvsa_attn_fwd_host(const void *qh, const void *kh, const void *vh,
         lvsa_set_error("NULL argument");
         return LVSA_EINVAL;
     }
+    lvsa_status_t dst = check_device(ix);
+    if (dst != LVSA_OK) return dst;
     cudaStream_t stream = (cudaStream_t)stream_;
     const size_t bytes = (size_t)ix->p.B * ix->N * ix->p.H * ix->p.d * elem_size(ix);
     const size_t lbytes = sizeof(float) * (size_t)ix->p.B * ix->p.H * ix->N;
-    // device staging buffers: one process-wide workspace per device, grown on demand, shared by
-    // every index handle (a per-step rebuild of the index must not re-allocate gigabytes)
+    // device staging buffers: one workspace per device, grown on demand, shared by every index
+    // handle (a per-step rebuild of the index must not re-allocate gigabytes)
     const size_t ab = (bytes + 255) & ~(size_t)255;
     const size_t need = 4 * ab + lbytes;
     std::lock_guard<std::mutex> lock(g_ws_mutex);
-    if (g_ws.ptr == nullptr || g_ws.cap < need || g_ws.device != ix->device) {
-        if (g_ws.ptr != nullptr) { cudaFree(g_ws.ptr); g_ws.ptr = nullptr; g_ws.cap = 0; }
-        LVSA_CUDA_TRY(cudaMalloc(&g_ws.ptr, need));
-        g_ws.cap = need; g_ws.device = ix->device;
+    HostWorkspace &ws = g_ws[ix->device];
+    if (ws.ptr == nullptr || ws.cap < need) {
+        if (ws.ptr != nullptr) { cudaFree(ws.ptr); ws.ptr = nullptr; ws.cap = 0; }
+        LVSA_CUDA_TRY(cudaMalloc(&ws.ptr, need));
+        ws.cap = need;
     }
-    uint8_t *wsp = static_cast<uint8_t *>(g_ws.ptr);
+    uint8_t *wsp = static_cast<uint8_t *>(ws.ptr);
     void *s_q = wsp, *s_k = wsp + ab, *s_v = wsp + 2 * ab, *s_o = wsp + 3 * ab;
     float *s_lse = reinterpret_cast<float *>(wsp + 4 * ab);
     // Pipelined path (CTA-pair kernel, bf16): heads are independent, so the call is cut into groups
     // of heads; the H2D copy of group g+1 and the D2H copy of group g-1 overlap the kernel of
-    // group g (strided 2-D copies of the [B*N, H*d] matrices, one column block per group).
-    static const int n_groups_env = getenv("LVSA_HOST_GROUPS") != nullptr ? atoi(getenv("LVSA_HOST_GROUPS")) : 16;
-    const int H = ix->p.H;
-    int G = n_groups_env < 1 ? 1 : n_groups_env;
-    if (G > H) G = H;
-    if (G > 1 && use_tcgen05(ix) && lvsa_attn_uses_pair_kernel(ix)) {
-        if (g_host.s_in == nullptr) {
-            LVSA_CUDA_TRY(cudaStreamCreateWithFlags(&g_host.s_in, cudaStreamNonBlocking));
-            LVSA_CUDA_TRY(cudaStreamCreateWithFlags(&g_host.s_out, cudaStreamNonBlocking));
+    // group g.  lvsa_params_t.host_groups: 0 = one head per group (at most MAXG groups), 1 = off.
+    int G = ix->p.host_groups == 0 ? HostPipe::MAXG : ix->p.host_groups;
+    if (G > ix->p.H) G = ix->p.H;
+    if (G > HostPipe::MAXG) G = HostPipe::MAXG;
+    const bool piped = G > 1 && use_tcgen05(ix) && lvsa_attn_uses_pair_kernel(ix);
+    HostPipe &hp = g_host[ix->device];
+    lvsa_status_t st;
+    if (piped) {
+        if (hp.ev_edge == nullptr) {
+            LVSA_CUDA_TRY(cudaStreamCreateWithFlags(&hp.s_in, cudaStreamNonBlocking));
+            LVSA_CUDA_TRY(cudaStreamCreateWithFlags(&hp.s_out, cudaStreamNonBlocking));
             for (int i = 0; i < HostPipe::MAXG; ++i) {
-                LVSA_CUDA_TRY(cudaEventCreateWithFlags(&g_host.ev_in[i], cudaEventDisableTiming));
-                LVSA_CUDA_TRY(cudaEventCreateWithFlags(&g_host.ev_c[i], cudaEventDisableTiming));
+                LVSA_CUDA_TRY(cudaEventCreateWithFlags(&hp.ev_in[i], cudaEventDisableTiming));
+                LVSA_CUDA_TRY(cudaEventCreateWithFlags(&hp.ev_c[i], cudaEventDisableTiming));
             }
-            LVSA_CUDA_TRY(cudaEventCreateWithFlags(&g_host.ev_edge, cudaEventDisableTiming));
+            LVSA_CUDA_TRY(cudaEventCreateWithFlags(&hp.ev_edge, cudaEventDisableTiming));
         }
-        if (G > HostPipe::MAXG) G = HostPipe::MAXG;
-        const size_t es = elem_size(ix), row = (size_t)H * ix->p.d * es;     // bytes per token (all heads)
-        const size_t rows = (size_t)ix->p.B * ix->N;
-        const int per = (H + G - 1) / G;
         index_touch_stream(ix, stream);
-        // copies start after whatever the caller already enqueued on `stream`
-        LVSA_CUDA_TRY(cudaEventRecord(g_host.ev_edge, stream));
-        LVSA_CUDA_TRY(cudaStreamWaitEvent(g_host.s_in, g_host.ev_edge, 0));
-        LVSA_CUDA_TRY(cudaStreamWaitEvent(g_host.s_out, g_host.ev_edge, 0));
-        int ng = 0;
-        for (int h0 = 0; h0 < H; h0 += per, ++ng) {
-            const int hc = h0 + per <= H ? per : H - h0;
-            const size_t off = (size_t)h0 * ix->p.d * es, width = (size_t)hc * ix->p.d * es;
-            const void *src[3] = {qh, kh, vh};
-            void *dst[3] = {s_q, s_k, s_v};
-            for (int t = 0; t < 3; ++t)
-                LVSA_CUDA_TRY(cudaMemcpy2DAsync((uint8_t *)dst[t] + off, row, (const uint8_t *)src[t] + off, row, width,
-                                                rows, cudaMemcpyHostToDevice, g_host.s_in));
-            LVSA_CUDA_TRY(cudaEventRecord(g_host.ev_in[ng], g_host.s_in));
-        }
-        ng = 0;
-        for (int h0 = 0; h0 < H; h0 += per, ++ng) {
-            const int hc = h0 + per <= H ? per : H - h0;
-            const size_t off = (size_t)h0 * ix->p.d * es, width = (size_t)hc * ix->p.d * es;
-            LVSA_CUDA_TRY(cudaStreamWaitEvent(stream, g_host.ev_in[ng], 0));
-            lvsa_status_t st = lvsa_attn_sm100_pair_launch_heads(ix, s_q, s_k, s_v, s_o, s_lse, h0, hc, stream);
-            if (st != LVSA_OK) return st;
-            LVSA_CUDA_TRY(cudaEventRecord(g_host.ev_c[ng], stream));
-            LVSA_CUDA_TRY(cudaStreamWaitEvent(g_host.s_out, g_host.ev_c[ng], 0));
-            LVSA_CUDA_TRY(cudaMemcpy2DAsync((uint8_t *)oh + off, row, (const uint8_t *)s_o + off, row, width, rows,
-                                            cudaMemcpyDeviceToHost, g_host.s_out));
-            if (lseh != nullptr)   // lse is [B, H, N]: heads h0.. of every batch are contiguous runs of hc * N floats
-                LVSA_CUDA_TRY(cudaMemcpy2DAsync(lseh + (size_t)h0 * ix->N, sizeof(float) * (size_t)H * ix->N,
-                                                s_lse + (size_t)h0 * ix->N, sizeof(float) * (size_t)H * ix->N,
-                                                sizeof(float) * (size_t)hc * ix->N, (size_t)ix->p.B,
-                                                cudaMemcpyDeviceToHost, g_host.s_out));
-        }
-        LVSA_CUDA_TRY(cudaEventRecord(g_host.ev_edge, g_host.s_out));
-        LVSA_CUDA_TRY(cudaStreamWaitEvent(stream, g_host.ev_edge, 0));
-        LVSA_CUDA_TRY(cudaStreamSynchronize(stream));
-        return LVSA_OK;
+        st = host_pipeline(ix, hp, G, qh, kh, vh, oh, lseh, s_q, s_k, s_v, s_o, s_lse, stream);
+    } else {
+        st = host_plain(ix, bytes, lbytes, qh, kh, vh, oh, lseh, s_q, s_k, s_v, s_o, s_lse, stream);
     }
-    LVSA_CUDA_TRY(cudaMemcpyAsync(s_q, qh, bytes, cudaMemcpyHostToDevice, stream));
-    LVSA_CUDA_TRY(cudaMemcpyAsync(s_k, kh, bytes, cudaMemcpyHostToDevice, stream));
-    LVSA_CUDA_TRY(cudaMemcpyAsync(s_v, vh, bytes, cudaMemcpyHostToDevice, stream));
-    lvsa_status_t st = lvsa_attn_fwd(s_q, s_k, s_v, ix, s_o, s_lse, stream);
-    if (st != LVSA_OK) return st;
-    LVSA_CUDA_TRY(cudaMemcpyAsync(oh, s_o, bytes, cudaMemcpyDeviceToHost, stream));
-    if (lseh != nullptr) LVSA_CUDA_TRY(cudaMemcpyAsync(lseh, s_lse, lbytes, cudaMemcpyDeviceToHost, stream));
-    LVSA_CUDA_TRY(cudaStreamSynchronize(stream));
+    // Whatever happened, nothing this call enqueued may still touch the caller's host buffers or the
+    // workspace when it returns: wait for all three streams, then report the first error.
+    const std::string first_error = st != LVSA_OK ? std::string(lvsa_last_error()) : std::string();
+    cudaError_t e_in = piped ? cudaStreamSynchronize(hp.s_in) : cudaSuccess;
+    cudaError_t e_main = cudaStreamSynchronize(stream);
+    cudaError_t e_out = piped ? cudaStreamSynchronize(hp.s_out) : cudaSuccess;
+    if (st != LVSA_OK) { lvsa_set_error(first_error); return st; }
+    LVSA_CUDA_TRY(e_in);
+    LVSA_CUDA_TRY(e_main);
+    LVSA_CUDA_TRY(e_out);
     return LVSA_OK;
 }
 
 void lvsa_workspace_release(void) {
     std::lock_guard<std::mutex> lock(g_ws_mutex);
-    if (g_ws.ptr != nullptr) cudaFree(g_ws.ptr);
-    g_ws.ptr = nullptr; g_ws.cap = 0; g_ws.device = -1;
+    int cur = -1;
+    cudaGetDevice(&cur);
+    for (int dev = 0; dev < LVSA_MAX_DEVICES; ++dev) {
+        if (g_ws[dev].ptr == nullptr) continue;
+        cudaSetDevice(dev);
+        cudaFree(g_ws[dev].ptr);
+        g_ws[dev].ptr = nullptr; g_ws[dev].cap = 0;
+    }
+    if (cur >= 0) cudaSetDevice(cur);
 }
 
 void lvsa_index_destroy(lvsa_index_t *ix) {
@@ -267,8 +325,9 @@ lvsa_status_t lvsa_index_info(const lvsa_index_t *ix, lvsa_index_info_t *info) {
     info->tile_q = p.tile_q; info->tile_k = p.tile_k; info->nq = ix->nq; info->nk = ix->nk;
     info->T_per = ix->T_per; info->phase = ix->phase; info->n_global = ix->n_global;
     info->words = ix->words; info->dtype = p.dtype; info->n_text = p.n_text;
-    info->initial_anchors = p.initial_anchors;
-    info->kernel = use_tcgen05(ix) ? LVSA_KERNEL_TCGEN05 : LVSA_KERNEL_SIMT;
+    info->initial_anchors = p.initial_anchors; info->layout = p.layout;
+    info->kernel = !use_tcgen05(ix) ? LVSA_KERNEL_SIMT
+                 : (p.kernel == LVSA_KERNEL_TCGEN05_V0 ? LVSA_KERNEL_TCGEN05_V0 : LVSA_KERNEL_TCGEN05);
     info->N = ix->N; info->nnz = ix->nnz; info->n_partial = ix->n_partial;
     info->n_items = ix->n_items; info->n_item_tiles = ix->n_item_tiles;
     return LVSA_OK;

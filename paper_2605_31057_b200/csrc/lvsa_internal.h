@@ -49,6 +49,16 @@ struct lvsa_index {
     int32_t *d_item_tiles = nullptr;  // [n_item_tiles], encoding above
 };
 
+// Element strides of the token, head and batch axes of q, k, v, out (d is contiguous):
+// NHD = [B, N, H, d], HND = [B, H, N, d] (lvsa_params_t.layout).
+struct lvsa_strides { long long n, h, b; };
+inline lvsa_strides lvsa_layout_strides(const lvsa_index *ix) {
+    const long long N = ix->N, H = ix->p.H, d = ix->p.d;
+    if (ix->p.layout == LVSA_LAYOUT_HND) return {d, N * d, H * N * d};
+    return {H * d, d, N * H * d};
+}
+constexpr int LVSA_MAX_DEVICES = 64;   // per-device one-time state is kept in arrays of this size
+
 void lvsa_set_error(const std::string &msg);
 lvsa_status_t lvsa_cuda_fail(cudaError_t e, const char *what);
 
@@ -70,11 +80,6 @@ lvsa_status_t lvsa_attn_simt_launch(const lvsa_index *ix, const void *q, const v
 lvsa_status_t lvsa_attn_sm100_launch(const lvsa_index *ix, const void *q, const void *k,
                                      const void *v, void *out, float *lse, cudaStream_t stream);
 int lvsa_attn_sm100_supported(const lvsa_index *ix);
-
-// lvsa_attn_sm100_ws.cu (warp-specialised persistent kernel, d = 128)
-lvsa_status_t lvsa_attn_sm100_ws_launch(const lvsa_index *ix, const void *q, const void *k,
-                                        const void *v, void *out, float *lse, cudaStream_t stream);
-lvsa_status_t lvsa_attn_sm100_ws_prepare(int device);
 
 // lvsa_attn_sm100_pair.cu (CTA-pair kernel, cta_group::2, d = 128)
 lvsa_status_t lvsa_attn_sm100_pair_launch(const lvsa_index *ix, const void *q, const void *k,

@@ -60,21 +60,30 @@ __device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
         : "memory");
     return done != 0;
 }
-// Bounded wait: a protocol bug traps (launch fails with an error) instead of hanging the GPU.
-#ifndef LVSA_MBAR_SPIN_LIMIT
-#define LVSA_MBAR_SPIN_LIMIT (1u << 17)
+// Bounded wait: a protocol bug traps (the launch fails with an error) instead of hanging the GPU.
+// The bound is wall time on the slow path only (%globaltimer, LVSA_MBAR_TIMEOUT_NS, 20 s by
+// default: orders of magnitude above any legitimate wait, also under a profiler's replay or heavy
+// throttling), not a spin count.  -DLVSA_MBAR_TIMEOUT_NS=0 compiles the bound out.
+#ifndef LVSA_MBAR_TIMEOUT_NS
+#define LVSA_MBAR_TIMEOUT_NS 20000000000ull
 #endif
+__device__ __forceinline__ uint64_t global_timer_ns() {
+    uint64_t t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+__device__ __forceinline__ void mbar_timeout(uint32_t bar, uint32_t parity) {
+#ifdef LVSA_DEBUG
+    printf("lvsa: mbarrier timeout: block %d thread %d barrier smem 0x%x parity %u\n", blockIdx.x,
+           threadIdx.x, bar, parity);
+#endif
+    __trap();
+}
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
     if (mbar_try_wait(bar, parity)) return;
-    uint32_t spins = 0;
+    const uint64_t t0 = global_timer_ns();
     while (!mbar_try_wait(bar, parity)) {
-        if (++spins > LVSA_MBAR_SPIN_LIMIT) {
-#ifdef LVSA_DEBUG
-            printf("lvsa: mbarrier timeout: block %d thread %d barrier smem 0x%x parity %u\n", blockIdx.x,
-                   threadIdx.x, bar, parity);
-#endif
-            __trap();
-        }
+        if (LVSA_MBAR_TIMEOUT_NS != 0ull && global_timer_ns() - t0 > LVSA_MBAR_TIMEOUT_NS) mbar_timeout(bar, parity);
     }
 }
 
@@ -271,15 +280,9 @@ __device__ __forceinline__ bool mbar_try_wait_cluster(uint32_t bar, uint32_t par
 }
 __device__ __forceinline__ void mbar_wait_cluster(uint32_t bar, uint32_t parity) {
     if (mbar_try_wait_cluster(bar, parity)) return;
-    uint32_t spins = 0;
+    const uint64_t t0 = global_timer_ns();
     while (!mbar_try_wait_cluster(bar, parity)) {
-        if (++spins > LVSA_MBAR_SPIN_LIMIT) {
-#ifdef LVSA_DEBUG
-            printf("lvsa: cluster mbarrier timeout: block %d thread %d barrier smem 0x%x parity %u\n", blockIdx.x,
-                   threadIdx.x, bar, parity);
-#endif
-            __trap();
-        }
+        if (LVSA_MBAR_TIMEOUT_NS != 0ull && global_timer_ns() - t0 > LVSA_MBAR_TIMEOUT_NS) mbar_timeout(bar, parity);
     }
 }
 

@@ -27,10 +27,27 @@ def test_library_exports_every_declared_symbol():
     assert "sm_100a" in binding.lvsa_version()
 
 
+def test_header_constants_match_binding():
+    """The enum values the binding hard-codes are the header's."""
+    src = open(os.path.join(ROOT, "include", "lvsa.h")).read()
+    vals = {k: int(v) for k, v in re.findall(r"\b(LVSA_[A-Z0-9_]+)\s*=\s*(-?\d+)", src)}
+    for name in ("KERNEL_AUTO", "KERNEL_SIMT", "KERNEL_TCGEN05", "KERNEL_TCGEN05_V0", "LAYOUT_NHD", "LAYOUT_HND",
+                 "DTYPE_BF16", "DTYPE_FP32", "TIE_LO", "TIE_HI", "TILE_FULL", "TILE_PARTIAL", "OK", "EINVAL",
+                 "EUNSUPPORTED", "ECUDA", "ENOMEM"):
+        assert vals["LVSA_" + name] == getattr(binding, name), name
+    # no debug hooks or environment switches in the product library (SURVEY.md section 5)
+    csrc = os.path.join(ROOT, "paper_2605_31057_b200", "csrc")
+    for f in os.listdir(csrc):
+        if f.endswith((".cu", ".cuh", ".h")):
+            assert "getenv" not in open(os.path.join(csrc, f)).read(), f
+    assert not hasattr(binding.lib(), "lvsa_debug_set_dump")
+
+
 def test_struct_sizes_match_header():
-    # 14 int32 + float + 2 int32; 21 int32 + pad + 5 int64
-    assert C.sizeof(binding.Params) == 17 * 4
+    # 14 int32 + float + 4 int32; 22 int32 + 5 int64 (include/lvsa.h)
+    assert C.sizeof(binding.Params) == 19 * 4
     assert C.sizeof(binding.IndexInfo) == 22 * 4 + 5 * 8
+    assert binding.IndexInfo.N.offset == 22 * 4
 
 
 def test_argument_validation_needs_no_gpu():
@@ -38,7 +55,8 @@ def test_argument_validation_needs_no_gpu():
            dict(T=4, P=4, H=1, d=64, anchors=-2), dict(T=4, P=4, H=1, d=64, step=-1),
            dict(T=4, P=4, H=1, d=64, layer=-1), dict(T=1 << 16, P=1 << 16, H=1, d=64),
            dict(T=4, P=4, H=1, d=64, tie_break=7), dict(T=4, P=4, H=1, d=64, initial_anchors=-1),
-           dict(T=4, P=4, H=1, d=64, n_text=-1)]
+           dict(T=4, P=4, H=1, d=64, n_text=-1), dict(T=4, P=4, H=1, d=64, layout=2),
+           dict(T=4, P=4, H=1, d=64, kernel=4), dict(T=4, P=4, H=1, d=64, host_groups=-1)]
     for kw in bad:
         with pytest.raises(binding.LvsaError) as ei:
             binding.lvsa_build_block_index_ex(**kw)
@@ -47,7 +65,8 @@ def test_argument_validation_needs_no_gpu():
         binding.lvsa_schedule_create(T=4, P=4, H=1, d=64, window=-1)
     assert ei.value.status == binding.EINVAL
     for kw in [dict(T=4, P=4, H=1, d=96), dict(T=4, P=4, H=1, d=128, tile_q=64, tile_k=64),
-               dict(T=4, P=4, H=1, d=64, dtype=binding.DTYPE_FP32, kernel=binding.KERNEL_TCGEN05)]:
+               dict(T=4, P=4, H=1, d=64, dtype=binding.DTYPE_FP32, kernel=binding.KERNEL_TCGEN05),
+               dict(T=4, P=4, H=1, d=128, dtype=binding.DTYPE_FP32, kernel=binding.KERNEL_TCGEN05_V0)]:
         with pytest.raises(binding.LvsaError) as ei:
             binding.lvsa_build_block_index_ex(**kw)
         assert ei.value.status == binding.EUNSUPPORTED, kw

@@ -40,6 +40,28 @@ def test_host_entry_point_matches_device_path_and_workspace_lifecycle():
     ix.destroy()
 
 
+@pytest.mark.parametrize("layout", ["nhd", "hnd"])
+@pytest.mark.parametrize("host_groups", [0, 1, 3, 16])
+def test_host_entry_point_head_groups(host_groups, layout):
+    """The pipelined host path with several heads per group and a short last group (H = 20: 16 groups of
+    2 heads -> 10 used; 3 groups of 7, 7, 6), B = 2 (strided lse copy with pitch H*N), lse requested, in
+    both memory orders; bitwise equal to the device path."""
+    w = inputs.Workload("host_b2_h20", 1, T=5, P=150, H=20, d=128, tile=128, W=1, a=2, B=2)
+    q, k, v = inputs.make_qkv(w, "cuda", torch.bfloat16)
+    kw = dict(host_groups=host_groups)
+    if layout == "hnd":
+        q, k, v = (x.transpose(1, 2).contiguous() for x in (q, k, v))
+        kw["layout"] = binding.LAYOUT_HND
+    ix = build_index(w, 1, **kw)
+    want, want_lse = gpu_attn(w, ix, q, k, v)
+    qh, kh, vh = (x.cpu().pin_memory() for x in (q, k, v))
+    oh = torch.full_like(qh, float("nan"))
+    lh = torch.full((w.B, w.H, w.N), float("nan"), dtype=torch.float32)
+    binding.lvsa_attn_fwd_host(qh, kh, vh, ix, oh, lh)
+    assert torch.equal(oh, want.cpu()) and torch.equal(lh, want_lse.cpu())
+    ix.destroy()
+
+
 def test_lse_is_optional_and_outputs_do_not_depend_on_it():
     w = inputs.WORKLOADS["small128"]
     q, k, v = inputs.make_qkv(w, "cuda", torch.bfloat16)
@@ -103,6 +125,9 @@ def test_attn_fwd_argument_errors():
     assert L.lvsa_attn_fwd(p(q), p(k), p(v), null, p(out), null, stream) == binding.EINVAL
     assert L.lvsa_attn_fwd(C.c_void_p(q.data_ptr() + 2), p(k), p(v), ix.handle, p(out), null, stream) == binding.EINVAL
     assert "aligned" in binding.lvsa_last_error()
+    lse = torch.empty((w.B, w.H, w.N + 1), device="cuda", dtype=torch.float32)
+    assert L.lvsa_attn_fwd(p(q), p(k), p(v), ix.handle, p(out), C.c_void_p(lse.data_ptr() + 2), stream) == binding.EINVAL
+    assert "lse" in binding.lvsa_last_error()
     assert L.lvsa_schedule_attn_fwd(null, 0, p(q), p(k), p(v), p(out), null, stream) == binding.EINVAL
     ix.destroy()
     ix.destroy()                      # second destroy of the Python wrapper is a no-op

@@ -13,6 +13,7 @@ from paper_2605_31057_b200 import binding, inputs
 pytestmark = pytest.mark.gpu
 
 KERNELS = {"tcgen05": dict(dtype=binding.DTYPE_BF16, kernel=binding.KERNEL_TCGEN05),
+           "tcgen05_v0": dict(dtype=binding.DTYPE_BF16, kernel=binding.KERNEL_TCGEN05_V0),
            "simt_bf16": dict(dtype=binding.DTYPE_BF16, kernel=binding.KERNEL_SIMT),
            "simt_fp32": dict(dtype=binding.DTYPE_FP32, kernel=binding.KERNEL_SIMT)}
 
@@ -26,14 +27,20 @@ def tol(kname):
     return BF16_MAX_ABS, BF16_MEAN_ABS, LSE_MAX_ABS_BF16
 
 
-def run_case(w, kname, steps, rows=None, layer=0, anchors=None, window=None, seed=None):
+def run_case(w, kname, steps, rows=None, layer=0, anchors=None, window=None, seed=None, hnd=False):
     torch_dtype = torch.float32 if kname == "simt_fp32" else torch.bfloat16
     q, k, v = inputs.make_qkv(w, "cuda", torch_dtype, seed=seed)
     rows = np.arange(w.N) if rows is None else rows
     mx, mean, lse_tol = tol(kname)
     for s in steps:
-        ix = build_index(w, s, layer, anchors=anchors, window=window, **KERNELS[kname])
-        out, lse = gpu_attn(w, ix, q, k, v)
+        if hnd:   # the same values stored [B, H, N, d]; the result comes back in that order too
+            ix = build_index(w, s, layer, anchors=anchors, window=window, layout=binding.LAYOUT_HND, **KERNELS[kname])
+            assert ix.info().layout == binding.LAYOUT_HND
+            out_t, lse = gpu_attn(w, ix, *(x.transpose(1, 2).contiguous() for x in (q, k, v)))
+            out = out_t.transpose(1, 2)
+        else:
+            ix = build_index(w, s, layer, anchors=anchors, window=window, **KERNELS[kname])
+            out, lse = gpu_attn(w, ix, q, k, v)
         for b in range(w.B):
             ref, ref_lse = oracle_attn(w, q, k, v, s, rows, anchors=anchors, window=window, b=b)
             st = compare(out, lse, ref, ref_lse, rows, b)
@@ -54,14 +61,22 @@ def test_tiny_all_steps_layers(kname):
         run_case(w, kname, w.steps if layer == 0 else w.steps[:4], layer=layer)
 
 
-@pytest.mark.parametrize("kname", ["simt_fp32", "simt_bf16", "tcgen05"])
+@pytest.mark.parametrize("kname", ["simt_fp32", "simt_bf16", "tcgen05", "tcgen05_v0"])
 @pytest.mark.parametrize("name", ["tiny_straddle", "small128"])
 def test_straddling_tiles_all_rows(name, kname):
     w = inputs.WORKLOADS[name]
     run_case(w, kname, w.steps[:5])
 
 
-@pytest.mark.parametrize("kname", ["simt_fp32", "tcgen05"])
+@pytest.mark.parametrize("kname", ["simt_fp32", "simt_bf16", "tcgen05", "tcgen05_v0"])
+@pytest.mark.parametrize("name", ["tiny_straddle", "small128", "small128_text", "batch2_d128"])
+def test_layout_hnd_all_rows(name, kname):
+    """lvsa_params_t.layout = HND: q, k, v, out stored [B, H, N, d] (PAPER.md:31 fixes only N = T*P)."""
+    w = inputs.WORKLOADS.get(name) or inputs.Workload("batch2_d128", 1, T=5, P=150, H=2, d=128, tile=128, W=1, a=2, B=2)
+    run_case(w, kname, w.steps[:2] if w.steps else (0, 1), hnd=True)
+
+
+@pytest.mark.parametrize("kname", ["simt_fp32", "tcgen05", "tcgen05_v0"])
 def test_edge_shapes(kname):
     W = inputs.Workload
     cases = [W("one_frame", 1, T=1, P=100, H=1, d=64, tile=64, W=0, a=0),           # single ragged tile
@@ -121,6 +136,26 @@ def test_large_configs_sampled_rows(name, n_rows):
         if ph not in seen:
             seen.add(ph); steps.append(s)
     run_case(w, "tcgen05", steps, rows=rows, layer=w.layers[0])
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("name", ["hv1.5_2x", "wan14b_6x"])
+def test_closed_form_probe_other_large_configs(name):
+    """P14 (Eq. 2) at full size on the other two large configs (T <= d holds: 65, 121)."""
+    w = inputs.WORKLOADS[name]
+    probe_check(w, "tcgen05", w.steps[:1])
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("name,window,anchors", [("hv1.5_2x", 2, 12),      # the exploratory HV budget C = 17
+                                                 ("wan1.3b_6x", 1, 18),    # W sweep of profiles/r01e: C = 21 held
+                                                 ("wan1.3b_6x", 5, 10)])
+def test_benched_variants_sampled_rows(name, window, anchors):
+    """Every configuration that bench.py / profiles/ report a time for is also a checked one: 1024
+    sampled rows (edge rows included) against the oracle at full size."""
+    w = inputs.WORKLOADS[name]
+    rows = inputs.sample_rows(w, n_uniform=768, n_edge=256)
+    run_case(w, "tcgen05", w.steps[1:2], rows=rows, layer=w.layers[0], anchors=anchors, window=window)
 
 
 @pytest.mark.slow

@@ -42,13 +42,19 @@ def structured_qkv(w, kind, seed=7):
     return q.to(torch.bfloat16), k.to(torch.bfloat16), v.to(torch.bfloat16)
 
 
+TC_KERNELS = {"tcgen05": binding.KERNEL_TCGEN05, "tcgen05_v0": binding.KERNEL_TCGEN05_V0}
+
+
+@pytest.mark.parametrize("kname", list(TC_KERNELS))
 @pytest.mark.parametrize("kind", ["growing", "shrinking", "one_hot", "offset"])
 @pytest.mark.parametrize("w", SHAPES, ids=lambda w: w.name)
-def test_structured_logits(w, kind):
+def test_structured_logits(w, kind, kname):
+    if kname == "tcgen05_v0" and w.d == 64:
+        pytest.skip("d = 64 runs the one-CTA kernel under both values")
     q, k, v = structured_qkv(w, kind)
     rows = np.arange(w.N)
     for s in (0, 1):
-        ix = build_index(w, s, dtype=binding.DTYPE_BF16, kernel=binding.KERNEL_TCGEN05)
+        ix = build_index(w, s, dtype=binding.DTYPE_BF16, kernel=TC_KERNELS[kname])
         out, lse = gpu_attn(w, ix, q, k, v)
         ref, ref_lse = oracle_attn(w, q, k, v, s, rows)
         st = compare(out, lse, ref, ref_lse, rows)
@@ -60,9 +66,10 @@ def test_structured_logits(w, kind):
         ix.destroy()
 
 
-def test_seeded_shape_sweep_d128():
-    """Odd sizes for the CTA-pair kernel: ragged tails, frames shorter / longer than a tile, odd
-    numbers of q tiles, batches, text tokens and dedicated anchors mixed."""
+@pytest.mark.parametrize("kname", list(TC_KERNELS))
+def test_seeded_shape_sweep_d128(kname):
+    """Odd sizes for the CTA-pair kernel (and the one-CTA kernel): ragged tails, frames shorter / longer
+    than a tile, odd numbers of q tiles, batches, text tokens and dedicated anchors mixed."""
     rng = np.random.default_rng(20260531)
     for case in range(24):
         T = int(rng.integers(1, 14))
@@ -74,7 +81,7 @@ def test_seeded_shape_sweep_d128():
         q, k, v = inputs.make_qkv(w, "cuda", torch.bfloat16, seed=1000 + case)
         rows = np.arange(w.N)
         s = int(rng.integers(0, 7))
-        ix = build_index(w, s, dtype=binding.DTYPE_BF16, kernel=binding.KERNEL_TCGEN05)
+        ix = build_index(w, s, dtype=binding.DTYPE_BF16, kernel=TC_KERNELS[kname])
         out, lse = gpu_attn(w, ix, q, k, v)
         for b in range(w.B):
             ref, ref_lse = oracle_attn(w, q, k, v, s, rows, b=b)

@@ -41,6 +41,31 @@ def test_worked_example_golden():
     assert np.array_equal(orc.pattern(8, 1, 2, 4).A, orc.pattern(8, 1, 2, 0).A)
 
 
+def test_a_bits_packing_pinned_by_hand():
+    """Pattern.a_bits() produces the expected value of bit-exact GPU comparisons, so its word / bit
+    order is pinned here without a device: the golden worked example packed by hand (bit x of word
+    x // 32 of row t set iff x in A(t), include/lvsa.h), and a T = 40 case that reaches the second
+    word, whose rows follow from the paper alone (a = 0: G is empty and A(t) is the clamped sliding
+    window of PAPER.md:68)."""
+    # s = 0 rows of tests/golden/worked_example_T8_W1_a2.txt, written as literals:
+    # {0,1,2,3,4} = 0x1f, {0,2,3,4,5} = 0x3d, {0,3,4,5,6} = 0x79, {0,4,5,6,7} = 0xf1
+    want0 = np.array([[0x1f], [0x1f], [0x1f], [0x3d], [0x3d], [0x79], [0xf1], [0xf1]], np.uint32)
+    got0 = orc.pattern(8, 1, 2, 0).a_bits()
+    assert got0.dtype == np.uint32 and got0.shape == (8, 1) and np.array_equal(got0, want0)
+    # and every row of the golden file, packed here with plain Python integers
+    for (s, t), want in read_golden_sets("worked_example_T8_W1_a2.txt"):
+        assert int(orc.pattern(8, 1, 2, s).a_bits()[t, 0]) == sum(1 << x for x in want), (s, t)
+    # T = 40, W = 2, no anchors: A(t) = [clamp(t-2), clamp(t-2)+4]; frames 30..34 straddle the words
+    p = orc.pattern(40, 2, 0, 0)
+    bits = p.a_bits()
+    assert bits.shape == (40, 2)
+    for t in range(40):
+        lo = max(0, min(t - 2, 40 - 5))
+        full = sum(1 << x for x in range(lo, lo + 5))
+        assert (int(bits[t, 0]), int(bits[t, 1])) == (full & 0xffffffff, full >> 32), t
+    assert (int(bits[32, 0]), int(bits[32, 1])) == (0xc0000000, 0x7)      # {30,31} | {32,33,34}
+
+
 def test_wan_budget_constants():
     # PAPER.md:60: C = (81-1)/4 + 1 = 21 latent frames; :110: T from 21 (1x) to 121 (6x)
     C = (81 - 1) // 4 + 1
