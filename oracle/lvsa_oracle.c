@@ -18,6 +18,7 @@
  *   O7  tile index = definition over token tiles         DESIGN.md reading R14 (paper silent)
  *   O8  Eq. 2 = softmax over the allowed keys, fp64
  *   O9  the same key set recovered through CSR + flags + element mask
+ *   O7b a second, frame-aligned kv tiling and its tile index     DESIGN.md reading R25 (cost only)
  *
  * Pins (tests/test_oracle_*.py, -m "not gpu"): Fig. 2 anchor sets, the closed
  * form |A(t)| = |G| + min(2W+1, T-|G|), |G^s| = ceil(T/T_per)
@@ -188,6 +189,84 @@ int64_t lvsa_oracle_tile_index(int T, int P, int n_text, int Bq, int Bk, const u
     return nnz;
 }
 
+/* ---- O7b: frame-aligned kv tiling (reading R25; the paper does not say how tokens map
+ * to blocks, and names further performance work as open) ----------- */
+/* Second tile definition, cost-only: the result of Eq. 2 does not depend on it.  The q tiles stay
+ * Bq tokens from token 0.  The kv tiles RESTART AT EVERY FRAME BOUNDARY: frame tau (P tokens; the
+ * text pseudo-frame has n_text) is cut into ceil(F/Bk) tiles, all Bk wide except the frame's last;
+ * tiles are numbered in token order.  So every kv tile lies inside ONE frame, and for a query row
+ * a tile is attended as a whole or not at all.
+ * Found by walking the tokens: a new tile starts at the first token of a frame and every Bk tokens
+ * after it.  col0[j] = first token of tile j, width[j] = its tokens.  Returns nk (cap: array size,
+ * -1 if too small; col0 == NULL: count only). */
+int64_t lvsa_oracle_kv_tiles_frame_aligned(int T, int P, int n_text, int Bk, int32_t *col0,
+                                           int32_t *width, int64_t cap)
+{
+    const int64_t N = (int64_t)T * P + n_text;
+    int64_t nk = 0, in_tile = 0, prev_frame = -1;
+    for (int64_t n = 0; n < N; ++n) {
+        const int64_t f = frame_of(n, T, P);
+        if (f != prev_frame || in_tile == Bk) {          /* open a new tile */
+            if (col0) { if (nk >= cap) return -1; col0[nk] = (int32_t)n; width[nk] = 0; }
+            ++nk; in_tile = 0; prev_frame = f;
+        }
+        if (width) width[nk - 1] += 1;
+        ++in_tile;
+    }
+    return nk;
+}
+
+/* Tile index over that tiling.  A kernel computes a kv tile over wpad = ceil(width/pad)*pad columns
+ * (pad = its column granularity; the columns past `width` are padding and never allowed):
+ *   K(i)      = sorted { j : exists valid row nq of q tile i with M(nq, col0[j]) }
+ *   flag(i,j) = 1 (PARTIAL) iff exists valid row nq of q tile i and c in [col0[j], col0[j]+wpad)
+ *               with c - col0[j] >= width[j] or not M(nq, c);  else 0 (FULL)
+ * M(nq, c) = A[frame(nq)][frame(c)].  Every column of the tile is walked (no use is made of the
+ * fact that they share a frame).  indices == NULL: count only.  Returns nnz or -1. */
+int64_t lvsa_oracle_tile_index_fa(int T, int P, int n_text, int Bq, int Bk, int pad, const uint8_t *A,
+                                  int32_t *indptr, int32_t *indices, uint8_t *flags, int64_t cap)
+{
+    const int64_t N = (int64_t)T * P + n_text;
+    const int Tf = T + (n_text > 0 ? 1 : 0);
+    const int64_t nq = (N + Bq - 1) / Bq;
+    const int64_t nk = lvsa_oracle_kv_tiles_frame_aligned(T, P, n_text, Bk, NULL, NULL, 0);
+    int32_t *col0 = (int32_t *)malloc(sizeof(int32_t) * (size_t)(nk + 1));
+    int32_t *width = (int32_t *)malloc(sizeof(int32_t) * (size_t)(nk + 1));
+    lvsa_oracle_kv_tiles_frame_aligned(T, P, n_text, Bk, col0, width, nk);
+    uint8_t *fq = (uint8_t *)malloc((size_t)Tf);
+    int *qf = (int *)malloc(sizeof(int) * (size_t)Tf);
+    int64_t nnz = 0;
+    for (int64_t i = 0; i < nq; ++i) {
+        if (indptr) indptr[i] = (int32_t)nnz;
+        /* the frames present among the valid rows of q tile i, as a list (found by walking the rows) */
+        memset(fq, 0, (size_t)Tf);
+        for (int64_t r = i * Bq; r < (i + 1) * Bq && r < N; ++r) fq[frame_of(r, T, P)] = 1;
+        int nqf = 0;
+        for (int tq = 0; tq < Tf; ++tq) if (fq[tq]) qf[nqf++] = tq;
+        for (int64_t j = 0; j < nk; ++j) {
+            const int64_t wpad = ((width[j] + pad - 1) / pad) * (int64_t)pad;
+            int any_allowed = 0, any_disallowed = 0;
+            for (int64_t c = col0[j]; c < col0[j] + wpad; ++c) {
+                if (c - col0[j] >= width[j]) { any_disallowed = 1; continue; }   /* padding column */
+                const int64_t fk = frame_of(c, T, P);
+                for (int x = 0; x < nqf; ++x) {
+                    if (A[(size_t)qf[x] * Tf + fk]) any_allowed = 1; else any_disallowed = 1;
+                }
+            }
+            if (!any_allowed) continue;
+            if (indices) {
+                if (nnz >= cap) { free(col0); free(width); free(fq); free(qf); return -1; }
+                indices[nnz] = (int32_t)j;
+                flags[nnz] = (uint8_t)any_disallowed;
+            }
+            ++nnz;
+        }
+    }
+    if (indptr) indptr[nq] = (int32_t)nnz;
+    free(col0); free(width); free(fq); free(qf);
+    return nnz;
+}
+
 /* ---- input decoding (not method arithmetic): element e of a tensor stored as fp32 or as
  * raw bf16 bit patterns, widened exactly to double ----------------------------------------- */
 static inline double ld_elem(const void *base, int is_bf16, int64_t e)
@@ -284,6 +363,43 @@ int lvsa_oracle_csr_keyset_equal(int T, int P, int n_text, int Bq, int Bk, const
         for (int64_t n = 0; n < N + Bk; ++n) {
             const int want = (n < N) ? Arow[frame_of(n, T, P)] : 0;
             if (via[n] != want) { ok = 0; break; }
+        }
+    }
+    free(via);
+    return ok;
+}
+
+/* O9 for an explicit kv tiling (col0, width per tile) and column granularity pad: FULL tiles
+ * contribute every one of their wpad columns without consulting M, PARTIAL tiles the columns inside
+ * `width` with M.  Returns 1 iff every key of every row in rows is contributed exactly once and
+ * nothing else is (which also catches overlapping or missing tiles). */
+int lvsa_oracle_csr_keyset_equal_tiles(int T, int P, int n_text, int Bq, int pad, const uint8_t *A,
+                                       const int32_t *col0, const int32_t *width,
+                                       const int32_t *indptr, const int32_t *indices,
+                                       const uint8_t *flags, const int64_t *rows, int64_t nrows)
+{
+    const int64_t N = (int64_t)T * P + n_text;
+    const int Tf = T + (n_text > 0 ? 1 : 0);
+    const int64_t slack = 4096;
+    uint8_t *via = (uint8_t *)malloc((size_t)(N + slack));
+    int ok = 1;
+    for (int64_t ri = 0; ri < nrows && ok; ++ri) {
+        const int64_t nqi = rows[ri];
+        const uint8_t *Arow = A + (size_t)frame_of(nqi, T, P) * Tf;
+        memset(via, 0, (size_t)(N + slack));
+        const int64_t i = nqi / Bq;
+        for (int32_t e = indptr[i]; e < indptr[i + 1]; ++e) {
+            const int64_t j = indices[e];
+            const int64_t wpad = ((width[j] + pad - 1) / pad) * (int64_t)pad;
+            if (wpad > slack) { ok = 0; break; }
+            for (int64_t c = col0[j]; c < col0[j] + wpad; ++c) {
+                if (flags[e]) { if (c - col0[j] < width[j] && c < N && Arow[frame_of(c, T, P)]) via[c] += 1; }
+                else          { via[c] += 1; }
+            }
+        }
+        for (int64_t n = 0; n < N + slack && ok; ++n) {
+            const int want = (n < N) ? Arow[frame_of(n, T, P)] : 0;
+            if (via[n] != want) ok = 0;
         }
     }
     free(via);

@@ -58,6 +58,8 @@ def lib() -> C.CDLL:
     if _lib is None:
         _lib = C.CDLL(build())
         _lib.lvsa_oracle_tile_index.restype = C.c_int64
+        _lib.lvsa_oracle_tile_index_fa.restype = C.c_int64
+        _lib.lvsa_oracle_kv_tiles_frame_aligned.restype = C.c_int64
         _lib.lvsa_oracle_time_rebuild.restype = C.c_double
     return _lib
 
@@ -133,6 +135,49 @@ def tile_index(T: int, P: int, Bq: int, Bk: int, A: np.ndarray, n_text: int = 0)
                                        _p(A), _p(indptr), _p(indices), _p(flags), C.c_int64(nnz))
     assert got == nnz
     return indptr, indices[:nnz], flags[:nnz]
+
+
+def kv_tiles_frame_aligned(T: int, P: int, Bk: int, n_text: int = 0):
+    """Frame-aligned kv tiling (reading R25): (col0, width) per kv tile, token order."""
+    nk = lib().lvsa_oracle_kv_tiles_frame_aligned(C.c_int(T), C.c_int(P), C.c_int(n_text), C.c_int(Bk),
+                                                  None, None, C.c_int64(0))
+    col0 = np.zeros(max(nk, 1), np.int32)
+    width = np.zeros(max(nk, 1), np.int32)
+    got = lib().lvsa_oracle_kv_tiles_frame_aligned(C.c_int(T), C.c_int(P), C.c_int(n_text), C.c_int(Bk),
+                                                   _p(col0), _p(width), C.c_int64(nk))
+    assert got == nk
+    return col0[:nk], width[:nk]
+
+
+def tile_index_fa(T: int, P: int, Bq: int, Bk: int, A: np.ndarray, n_text: int = 0, pad: int = 32):
+    """CSR (indptr, indices, flags) over the frame-aligned kv tiling; flags 1 = PARTIAL (some row of
+    the q tile does not attend to the tile's frame, or the tile is narrower than its padded width)."""
+    A = np.ascontiguousarray(A, np.uint8)
+    assert A.shape == (T + (n_text > 0), T + (n_text > 0))
+    N = T * P + n_text
+    nq = (N + Bq - 1) // Bq
+    indptr = np.zeros(nq + 1, np.int32)
+    args = (C.c_int(T), C.c_int(P), C.c_int(n_text), C.c_int(Bq), C.c_int(Bk), C.c_int(pad), _p(A), _p(indptr))
+    nnz = lib().lvsa_oracle_tile_index_fa(*args, None, None, C.c_int64(0))
+    indices = np.zeros(max(nnz, 1), np.int32)
+    flags = np.zeros(max(nnz, 1), np.uint8)
+    got = lib().lvsa_oracle_tile_index_fa(*args, _p(indices), _p(flags), C.c_int64(nnz))
+    assert got == nnz
+    return indptr, indices[:nnz], flags[:nnz]
+
+
+def csr_keyset_equal_tiles(T, P, Bq, A, col0, width, indptr, indices, flags, rows, n_text: int = 0,
+                           pad: int = 32) -> bool:
+    A = np.ascontiguousarray(A, np.uint8)
+    rows = np.ascontiguousarray(rows, np.int64)
+    col0 = np.ascontiguousarray(col0, np.int32)
+    width = np.ascontiguousarray(width, np.int32)
+    indptr = np.ascontiguousarray(indptr, np.int32)
+    indices = np.ascontiguousarray(indices, np.int32)
+    flags = np.ascontiguousarray(flags, np.uint8)
+    return bool(lib().lvsa_oracle_csr_keyset_equal_tiles(
+        C.c_int(T), C.c_int(P), C.c_int(n_text), C.c_int(Bq), C.c_int(pad), _p(A), _p(col0), _p(width),
+        _p(indptr), _p(indices), _p(flags), _p(rows), C.c_int64(rows.size)))
 
 
 def _as_input(x) -> tuple[np.ndarray, int]:
