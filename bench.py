@@ -95,18 +95,20 @@ class ClockSampler:
 
 
 def ncu_traffic(workload: str):
-    """dram__bytes_read.sum + dram__bytes_write.sum of one attention launch, from the committed
-    `ncu --set full` capture (profiles/traffic.csv names the summary it came from); never measured
-    live, None when no capture exists for this workload."""
+    """dram__bytes_read.sum + dram__bytes_write.sum of one attention launch and the tensor-pipe busy
+    percentage (sm__pipe_tensor_cycles_active), from the committed `ncu --set full` capture of this
+    workload (profiles/traffic.csv names the summary they came from); never measured live, None when
+    no capture exists for this workload."""
     import csv
     p = os.path.join(ROOT, "profiles", "traffic.csv")
     if not os.path.exists(p):
-        return None, None
+        return None, None, None
     with open(p, newline="") as f:
         for row in csv.DictReader(f):
             if row["workload"] == workload:
-                return int(row["dram_bytes_per_launch"]), row["source"]
-    return None, None
+                pct = row.get("tensor_pipe_active_pct")
+                return int(row["dram_bytes_per_launch"]), row["source"], (float(pct) if pct else None)
+    return None, None, None
 
 
 def dist_setup(n_gpus: int):
@@ -137,16 +139,22 @@ def run_ours(args):
     stream = torch.cuda.current_stream()
     steps_cycle = list(w.steps) if w.steps else [0]
 
-    def build(s):
+    def build(s, **kw):
         return binding.lvsa_build_block_index_ex(
             stream=stream.cuda_stream, T=w.T, P=w.P, H=w.H, d=w.d, B=w.B, window=w.W, anchors=w.a,
-            step=s, layer=w.layers[0] if w.layers else 0)
+            step=s, layer=w.layers[0] if w.layers else 0, n_text=w.n_text, initial_anchors=w.k0, **kw)
 
-    # nnz per distinct step of the cycle (lvsa_index_info synchronises, so it stays out of the timed region)
-    nnz_of = {}
+    def tile_flop(kept_cols):
+        """Computed-tile work: S = Q K^T and O += P V over tile_q rows x the kept kv columns."""
+        return float(kept_cols) * w.tile * 4.0 * w.d * w.H * w.B
+
+    # kept tiles / columns per distinct step of the cycle (lvsa_index_info synchronises, so it stays
+    # out of the timed region)
+    nnz_of, cols_of = {}, {}
     for s in sorted(set(steps_cycle)):
         ix0 = build(s)
-        nnz_of[s] = ix0.info().nnz
+        i0 = ix0.info()
+        nnz_of[s], cols_of[s] = i0.nnz, i0.kept_cols
         ix0.destroy()
 
     def one_step(i):
@@ -191,14 +199,14 @@ def run_ours(args):
     total_ms = e0.elapsed_time(e1)
     launches_per_step = 4 + attn_launches   # 4 index-builder kernels + attention
     step_nnz = [nnz_of[steps_cycle[i % len(steps_cycle)]] for i in range(args.steps)]
-    tile_flops = sum(float(n) * w.H * w.B * 4.0 * w.tile * w.tile * w.d for n in step_nnz)
+    tile_flops = sum(tile_flop(cols_of[steps_cycle[i % len(steps_cycle)]]) for i in range(args.steps))
     nnz_mean = float(np.mean(step_nnz))
     kern_ms = float(np.mean([a.elapsed_time(b) for a, b in zip(ka, kb)]))     # sustained, inside the step
     kern_flops = tile_flops / args.steps
 
     # ---- the same kernel timed alone after an idle gap (burst clocks, no power cap yet): min of 5
     ix_k = build(steps_cycle[min(1, len(steps_cycle) - 1)])
-    burst_flops = float(nnz_of[steps_cycle[min(1, len(steps_cycle) - 1)]]) * w.H * w.B * 4.0 * w.tile * w.tile * w.d
+    burst_flops = tile_flop(cols_of[steps_cycle[min(1, len(steps_cycle) - 1)]])
     burst = []
     for _ in range(5):
         torch.cuda.synchronize()
@@ -210,6 +218,32 @@ def run_ours(args):
         torch.cuda.synchronize()
         burst.append(k0.elapsed_time(k1))
     burst_ms = float(min(burst))
+
+    # ---- the frame-aligned kv tiling (row f4, reading R25) on the same inputs: same timing recipe as
+    # the headline kernel (back to back inside a loop, and alone after an idle gap)
+    fa_line = None
+    if rank == 0 and not args.no_dense:
+        s_fa = steps_cycle[min(1, len(steps_cycle) - 1)]
+        ix_fa = build(s_fa, kv_tiling=binding.KV_TILES_FRAME_ALIGNED)
+        i_fa = ix_fa.info()
+
+        def time_loop(ix, n):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            for _ in range(3):
+                binding.lvsa_attn_fwd(q, k, v, ix, out, lse, stream.cuda_stream)
+            a.record(stream)
+            for _ in range(n):
+                binding.lvsa_attn_fwd(q, k, v, ix, out, lse, stream.cuda_stream)
+            b.record(stream)
+            torch.cuda.synchronize()
+            return a.elapsed_time(b) / n
+        n_fa = max(5, min(args.steps, 20))
+        fa_ms, tok_ms = time_loop(ix_fa, n_fa), time_loop(ix_k, n_fa)
+        fa_line = {"ms": round(fa_ms, 4), "ms_token0_same_loop": round(tok_ms, 4), "nnz": int(i_fa.nnz),
+                   "kept_cols": int(i_fa.kept_cols), "kept_cols_token0": int(cols_of[s_fa]),
+                   "tflops_computed": round(tile_flop(i_fa.kept_cols) / (fa_ms * 1e-3) / 1e12, 1),
+                   "note": "fewer computed columns, more tile visits: the kernel's time follows the tile visits (DESIGN.md 7.2c)"}
+        ix_fa.destroy()
 
     # ---- index build alone (a1-a5): 4 kernels, enqueue only; device time by events, host time by clock
     torch.cuda.synchronize()
@@ -279,6 +313,7 @@ def run_ours(args):
         torch.cuda.synchronize()
         dense_ms = d0.elapsed_time(d1)
         dense_nnz = ixd.info().nnz
+        dense_cols = ixd.info().kept_cols
         ixd.destroy()
         # restore the LVSA result in `out`
         binding.lvsa_attn_fwd(q, k, v, ix_k, out, lse, stream.cuda_stream)
@@ -302,7 +337,7 @@ def run_ours(args):
             ixh = build(s_i)
             binding.lvsa_attn_fwd_host(qh, kh, vh, ixh, oh, lh, stream.cuda_stream)   # H2D + kernel + D2H + sync
             ixh.destroy()
-            fl_e2e += float(nnz_of[s_i]) * w.H * w.B * 4.0 * w.tile * w.tile * w.d
+            fl_e2e += tile_flop(cols_of[s_i])
         h1.record(stream)
         barrier()
         e2e_ms = h0.elapsed_time(h1) / n_e2e
@@ -338,7 +373,16 @@ def run_ours(args):
         peak_sus = pk["bf16_tflops_sustained"]
         achieved = kern_flops / (kern_ms * 1e-3) / 1e12
         burst_tf = burst_flops / (burst_ms * 1e-3) / 1e12
-        traffic, traffic_src = ncu_traffic(args.workload)
+        traffic, traffic_src, tensor_pct = ncu_traffic(args.workload)
+        # the exact Eq. 2 work of the same calls (4 d flop per attended key and query row), from the
+        # frame-level pattern the library reports (a_bits): what the computed tiles are an upper bound of
+        ix_e = build(steps_cycle[0])
+        ab = ix_e.copy_host().a_bits
+        ix_e.destroy()
+        Tf = ab.shape[0]
+        frame_len = np.array([w.P] * w.T + ([w.n_text] if w.n_text else []), dtype=np.float64)
+        bits = ((ab[:, :, None] >> np.arange(32, dtype=np.uint32)[None, None, :]) & 1).reshape(Tf, -1)[:, :Tf]
+        useful = float((frame_len[:, None] * bits * frame_len[None, :]).sum()) * 4.0 * w.d * w.H * w.B
         line = {
             "metric": METRIC, "value": round(value, 2), "unit": UNIT, "n_gpus": world,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": round(ms_step, 4),
@@ -350,6 +394,8 @@ def run_ours(args):
                        "l2": "inputs (3 x %.0f MB) exceed the 126 MB L2; no flush" % (q.numel() * 2 / 1e6),
                        "parallelism": "replicas only (one independent call per GPU)" if world > 1 else "1 GPU"},
             "ms_per_attention_call": round(kern_ms, 4),
+            "tflops_exact_eq2_work": round(useful / (kern_ms * 1e-3) / 1e12, 1),
+            "computed_over_exact_work": round(tile_flop(cols_of[steps_cycle[0]]) / useful, 4),
             "index_build_us": round(build_us, 1), "index_build_host_enqueue_us": round(build_host_us, 1),
             "pct_of_peak": {"sustained_kernel_vs_sustained_peak_%.1f" % pk["bf16_tflops_sustained"]: round(100 * achieved / pk["bf16_tflops_sustained"], 2),
                             "burst_kernel_vs_burst_peak_%.1f" % pk["bf16_tflops"]: round(100 * burst_tf / pk["bf16_tflops"], 2),
@@ -358,7 +404,8 @@ def run_ours(args):
             "all_tiles": None if dense_ms is None else {
                 "ms": round(dense_ms, 3), "nnz": int(dense_nnz),
                 "speedup_lvsa_vs_all_tiles": round(dense_ms / kern_ms, 3),
-                "tflops": round(float(dense_nnz) * w.H * w.B * 4.0 * w.tile * w.tile * w.d / (dense_ms * 1e-3) / 1e12, 1)},
+                "tflops": round(tile_flop(dense_cols) / (dense_ms * 1e-3) / 1e12, 1)},
+            "frame_aligned_kv_tiles": fa_line,
             "schedule": sched_line,
             "roofline": {"bound": "tensor", "achieved": round(achieved, 2), "peak": peak_sus,
                          "unit": "TFLOP/s", "frac": round(achieved / peak_sus, 4), "traffic": traffic,
@@ -367,6 +414,8 @@ def run_ours(args):
                          "kernel": "lvsa_attn_sm100_pair_kernel", "flops_per_launch": kern_flops,
                          "ms_per_launch": round(kern_ms, 4),
                          "traffic_source": traffic_src,
+                         "tensor_pipe_active_pct": tensor_pct,
+                         "frac_sustained_time_vs_burst_peak": round(achieved / pk["bf16_tflops"], 4),
                          "burst": {"ms_per_launch": round(burst_ms, 4), "achieved": round(burst_tf, 2),
                                    "peak": pk["bf16_tflops"], "frac": round(burst_tf / pk["bf16_tflops"], 4),
                                    "how": "one launch after a 0.25 s idle gap, min of 5, vs the burst peak"}},
@@ -420,14 +469,16 @@ def run_reference(args):
         fl += last["value"] * 1e12 * last["seconds"]
     sec = time.perf_counter() - t0
     val = fl / sec / 1e12
-    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+    ref_unit = "TFLOP/s (fp64, exact Eq. 2 flops)"
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": ref_unit, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": sec * 1e3 / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
             "data": "synthetic (same seeded tensors as the CUDA arm)",
-            "config": {"workload": args.workload, "T": w.T, "P": w.P, "N": w.N, "H": w.H, "d": w.d},
-            "cpu_baseline": {"value": val, "unit": UNIT, "cores": last["cores"], "kind": "oracle",
+            "config": {"workload": args.workload, "T": w.T, "P": w.P, "N": w.N, "H": w.H, "d": w.d,
+                       "B": w.B, "tile": w.tile, "window": w.W, "anchors": w.a, "steps_cycled": steps_cycle},
+            "cpu_baseline": {"value": val, "unit": ref_unit, "cores": last["cores"], "kind": "oracle",
                              "sample": f"each step: {last['sample']} (exact Eq. 2 flops, fp64)"},
-            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "e2e": {"value": val, "unit": ref_unit, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
 

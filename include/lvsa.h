@@ -46,6 +46,17 @@ enum { LVSA_KERNEL_AUTO = 0, LVSA_KERNEL_SIMT = 1, LVSA_KERNEL_TCGEN05 = 2, LVSA
 /* Memory order of q, k, v, out (PAPER.md:31 fixes only N = T*P, not the order of the axes):
  * NHD = [B, N, H, d] (default), HND = [B, H, N, d]; d is always fastest.  lse is [B, H, N] in both. */
 enum { LVSA_LAYOUT_NHD = 0, LVSA_LAYOUT_HND = 1 };
+/* How the key/value tokens are cut into kv tiles (cost only: the result is Eq. 2 either way; the paper
+ * does not say how tokens map to blocks):
+ *   TOKEN0        : tile j = tokens [j*tile_k, (j+1)*tile_k), from token 0 (reading R14).
+ *   FRAME_ALIGNED : kv tiles restart at every frame boundary: a frame of P tokens (the text pseudo-frame:
+ *                   n_text) is cut into ceil(P/tile_k) tiles, all tile_k wide except the frame's last
+ *                   (reading R25).  Every kv tile then lies inside one frame, so a query row attends to a
+ *                   tile as a whole or not at all; the kernels compute a tile over its width rounded up
+ *                   to LVSA_KV_PAD columns.  Accepted by the CTA-pair kernel (d = 128) and the SIMT
+ *                   kernel; LVSA_EUNSUPPORTED with the one-CTA-per-item tcgen05 kernel (d = 64, _V0). */
+enum { LVSA_KV_TILES_TOKEN0 = 0, LVSA_KV_TILES_FRAME_ALIGNED = 1 };
+#define LVSA_KV_PAD 32 /* column granularity of a narrow kv tile (FRAME_ALIGNED) */
 
 /* Parameters of lvsa_build_block_index_ex.  Zero means "default" where a default is named. */
 typedef struct lvsa_params {
@@ -75,6 +86,7 @@ typedef struct lvsa_params {
     int32_t layout;     /* LVSA_LAYOUT_NHD (default) or LVSA_LAYOUT_HND: memory order of q,k,v,out     */
     int32_t host_groups;/* lvsa_attn_fwd_host only: number of head groups the call is pipelined over
                            (0 = default: one head per group, at most 16 groups; 1 = unpipelined)      */
+    int32_t kv_tiling;  /* LVSA_KV_TILES_TOKEN0 (default) or LVSA_KV_TILES_FRAME_ALIGNED               */
 } lvsa_params_t;
 
 typedef struct lvsa_index_info {
@@ -90,8 +102,14 @@ typedef struct lvsa_index_info {
     int32_t n_text;          /* text tokens after the video tokens (R23)                        */
     int32_t initial_anchors; /* dedicated initial anchors k0 (R22)                              */
     int32_t layout;          /* LVSA_LAYOUT_*                                                   */
+    int32_t kv_tiling;       /* LVSA_KV_TILES_*                                                 */
+    int32_t reserved0;       /* 0                                                               */
     int64_t N;               /* T*P + n_text                                                    */
     int64_t nnz;             /* kept (q tile, kv tile) pairs                                    */
+    int64_t kept_cols;       /* sum over the kept pairs of the kv columns a kernel computes for
+                                them (tile_k, or the width rounded up to LVSA_KV_PAD for a narrow
+                                FRAME_ALIGNED tile): computed work = tile_q * kept_cols * 4d flop
+                                per head and batch                                              */
     int64_t n_partial;       /* of which PARTIAL                                                */
     int64_t n_items;         /* work items of the attention kernel (q-tile groups)              */
     int64_t n_item_tiles;    /* kv-tile visits over all items (>= nnz / rows-per-item ratio)    */
@@ -101,7 +119,8 @@ typedef struct lvsa_index_info {
  * lvsa_build_block_index — steps a1..a5 of the hot path on the GPU (Alg. 1
  * :74-89, Eq. 3 :97, Def. 2 :49; tile mapping per DESIGN.md reading R14).
  * Builds, for denoising step `step`, the per-frame attended sets A(t) and the CSR of kept
- * kv tiles per q tile (tile = 128 tokens for d = 128, 64 for d = 64; tiles start at token 0):
+ * kv tiles per q tile (tile = 128 tokens for d = 128, 64 for d = 64; q tiles start at token 0, kv
+ * tiles too unless lvsa_params_t.kv_tiling says FRAME_ALIGNED):
  *   indptr[nq+1], indices[nnz] ascending within a q tile, flags[nnz] in {FULL, PARTIAL}.
  * A kv tile is kept iff some (valid query row, valid key column) pair is allowed; it is PARTIAL
  * iff some (valid row, column of the tile) pair is not (frame not attended, or column >= N).
@@ -199,6 +218,11 @@ lvsa_status_t lvsa_index_info(const lvsa_index_t *index, lvsa_index_info_t *info
 lvsa_status_t lvsa_index_copy_host(const lvsa_index_t *index, int32_t *indptr, int32_t *indices,
                                    uint8_t *flags, int32_t *w_lo, int32_t *w_hi,
                                    uint32_t *a_bits);
+
+/* The kv tiling of the index as HOST arrays of nk entries each (lvsa_index_info: nk): col0[j] = first
+ * token of kv tile j, width[j] = its tokens (<= tile_k).  Either pointer may be NULL.  Pure host
+ * arithmetic from the parameters; no device work. */
+lvsa_status_t lvsa_index_copy_kv_tiles(const lvsa_index_t *index, int32_t *col0, int32_t *width);
 
 /* Number of kernels lvsa_attn_fwd enqueues per call for this index (bench.py's gpu_launches). */
 int lvsa_attn_fwd_launches(const lvsa_index_t *index);

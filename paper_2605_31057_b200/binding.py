@@ -22,6 +22,8 @@ TIE_LO, TIE_HI = 0, 1
 DTYPE_BF16, DTYPE_FP32 = 0, 1
 KERNEL_AUTO, KERNEL_SIMT, KERNEL_TCGEN05, KERNEL_TCGEN05_V0 = 0, 1, 2, 3
 LAYOUT_NHD, LAYOUT_HND = 0, 1
+KV_TILES_TOKEN0, KV_TILES_FRAME_ALIGNED = 0, 1
+KV_PAD = 32
 OK, EINVAL, EUNSUPPORTED, ECUDA, ENOMEM = 0, 1, 2, 3, 4
 
 
@@ -38,20 +40,21 @@ class Params(C.Structure):
                                                      ("initial_anchors", C.c_int32),
                                                      ("n_text", C.c_int32),
                                                      ("layout", C.c_int32),
-                                                     ("host_groups", C.c_int32)]
+                                                     ("host_groups", C.c_int32),
+                                                     ("kv_tiling", C.c_int32)]
 
 
 class IndexInfo(C.Structure):
     _fields_ = [(n, C.c_int32) for n in
                 ("T", "P", "H", "d", "B", "window", "anchors", "step", "layer", "tile_q", "tile_k",
                  "nq", "nk", "T_per", "phase", "n_global", "words", "dtype", "kernel", "n_text",
-                 "initial_anchors", "layout")] + \
-               [(n, C.c_int64) for n in ("N", "nnz", "n_partial", "n_items", "n_item_tiles")]
+                 "initial_anchors", "layout", "kv_tiling", "reserved0")] + \
+               [(n, C.c_int64) for n in ("N", "nnz", "kept_cols", "n_partial", "n_items", "n_item_tiles")]
 
 
 EXPORTS = ("lvsa_build_block_index", "lvsa_build_block_index_ex", "lvsa_attn_fwd",
            "lvsa_attn_fwd_host", "lvsa_index_destroy", "lvsa_index_info", "lvsa_index_copy_host",
-           "lvsa_attn_fwd_launches", "lvsa_workspace_release", "lvsa_schedule_create",
+           "lvsa_index_copy_kv_tiles", "lvsa_attn_fwd_launches", "lvsa_workspace_release", "lvsa_schedule_create",
            "lvsa_schedule_num_phases", "lvsa_schedule_index", "lvsa_schedule_attn_fwd", "lvsa_schedule_destroy", "lvsa_last_error", "lvsa_version")
 
 _lib = None
@@ -77,6 +80,8 @@ def lib() -> C.CDLL:
         L.lvsa_index_info.argtypes = [C.c_void_p, C.POINTER(IndexInfo)]
         L.lvsa_index_copy_host.restype = C.c_int
         L.lvsa_index_copy_host.argtypes = [C.c_void_p] * 7
+        L.lvsa_index_copy_kv_tiles.restype = C.c_int
+        L.lvsa_index_copy_kv_tiles.argtypes = [C.c_void_p] * 3
         L.lvsa_attn_fwd_launches.restype = C.c_int
         L.lvsa_attn_fwd_launches.argtypes = [C.c_void_p]
         L.lvsa_workspace_release.restype = None
@@ -150,6 +155,14 @@ class BlockIndex:
         _check(lib().lvsa_index_copy_host(self.handle, ptr(indptr), ptr(indices), ptr(flags),
                                           ptr(w_lo), ptr(w_hi), ptr(a_bits)))
         return HostIndex(indptr, indices, flags, w_lo, w_hi, a_bits)
+
+    def kv_tiles(self):
+        """(col0, width) of every kv tile of the index's tiling (host arithmetic in the library)."""
+        nk = self.info().nk
+        col0, width = np.zeros(nk, np.int32), np.zeros(nk, np.int32)
+        _check(lib().lvsa_index_copy_kv_tiles(self.handle, col0.ctypes.data_as(C.c_void_p),
+                                              width.ctypes.data_as(C.c_void_p)))
+        return col0, width
 
     def launches(self) -> int:
         return int(lib().lvsa_attn_fwd_launches(self.handle))

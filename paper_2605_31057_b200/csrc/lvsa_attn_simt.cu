@@ -30,7 +30,7 @@ lvsa_attn_simt_kernel(const T *__restrict__ q, const T *__restrict__ k, const T 
                       const int32_t *__restrict__ indptr, const int32_t *__restrict__ indices,
                       const uint8_t *__restrict__ flags, const uint32_t *__restrict__ a_bits,
                       int words, long long N, int P, int Tf, int H, long long sn, long long sh, long long sb,
-                      float scale) {
+                      int aligned, int Tv, float scale) {
     constexpr int R = BT / SIMT_WARPS;  // rows per warp
     constexpr int CH = D / 32;          // output channels per lane
     constexpr int KS = D + 1;           // padded K row (lane c reads row c: conflict-free)
@@ -65,12 +65,15 @@ lvsa_attn_simt_kernel(const T *__restrict__ q, const T *__restrict__ k, const T 
     for (int e = e0; e < e1; ++e) {
         const int j = indices[e];
         const bool partial = flags[e] != LVSA_TILE_FULL;
-        const long long col0 = (long long)j * BT;
+        // geometry of kv tile j under the index's tiling (token-0 tiles or frame-aligned tiles, R25)
+        const lvsa_kv_tile kt = lvsa_kv_tile_of(j, aligned, BT, P, Tv, N);
+        const long long col0 = kt.c0;
+        const int nchunks = (kt.width + 31) / 32;   // 32-column chunks that hold valid columns
         __syncthreads();
         for (int x = tid; x < BT * D; x += blockDim.x) {
             const int r = x / D, c = x % D;
             const long long n = col0 + r;
-            const bool ok = n < N;
+            const bool ok = r < kt.width;
             Ks[r * KS + c] = ok ? to_f32<T>(kb[(size_t)n * tok_stride + c]) : 0.f;
             Vs[r * D + c] = ok ? to_f32<T>(vb[(size_t)n * tok_stride + c]) : 0.f;
         }
@@ -82,7 +85,7 @@ lvsa_attn_simt_kernel(const T *__restrict__ q, const T *__restrict__ k, const T 
             if (nq >= N) continue;  // warp-uniform
             const uint32_t *arow = a_bits + (size_t)min((int)(nq / P), Tf - 1) * words;   // text rows: frame Tf-1
             const float *qrow = Qs + rl * D;
-            for (int cc = 0; cc < BT / 32; ++cc) {
+            for (int cc = 0; cc < nchunks; ++cc) {
                 const int cl = cc * 32 + lane;
                 const float *krow = Ks + cl * KS;
                 float s = 0.f;
@@ -91,7 +94,7 @@ lvsa_attn_simt_kernel(const T *__restrict__ q, const T *__restrict__ k, const T 
                 s *= scale;
                 if (partial) {
                     const long long nk_ = col0 + cl;
-                    bool ok = nk_ < N;
+                    bool ok = cl < kt.width;
                     if (ok) { const int f = min((int)(nk_ / P), Tf - 1); ok = (arow[f >> 5] >> (f & 31)) & 1u; }
                     if (!ok) s = -INFINITY;
                 }
@@ -145,7 +148,8 @@ lvsa_status_t launch(const lvsa_index *ix, const void *q, const void *k, const v
     dim3 grid(ix->nq, ix->p.H, ix->p.B);
     kern<<<grid, SIMT_WARPS * 32, smem, stream>>>(
         (const T *)q, (const T *)k, (const T *)v, (T *)out, lse, ix->d_indptr, ix->d_indices,
-        ix->d_flags, ix->d_abits, ix->words, (long long)ix->N, ix->p.P, ix->Tf, ix->p.H, sd.n, sd.h, sd.b, scale);
+        ix->d_flags, ix->d_abits, ix->words, (long long)ix->N, ix->p.P, ix->Tf, ix->p.H, sd.n, sd.h, sd.b,
+        ix->p.kv_tiling == LVSA_KV_TILES_FRAME_ALIGNED, ix->p.T, scale);
     LVSA_CUDA_TRY(cudaGetLastError());
     return LVSA_OK;
 }

@@ -40,9 +40,6 @@ constexpr int SPAN_BYTES = BT * 128;            // 16 KB: [128 rows][128 B] swiz
 constexpr int STAGE_BYTES = 16384;              // half a K tile (64 rows x 256 B) or half a V tile (128 rows x 128 B)
 constexpr int NTHREADS = 384;
 constexpr float RESCALE_THRESHOLD = 8.0f;       // log2 units
-#ifndef LVSA_POLY_PAIRS
-#define LVSA_POLY_PAIRS 0
-#endif
 #ifndef LVSA_PAIR_STAGES
 #define LVSA_PAIR_STAGES 10
 #endif
@@ -71,15 +68,25 @@ __device__ __forceinline__ uint32_t range_mask32(int lo, int hi, int w) {
 template <int REGS> __device__ __forceinline__ void reg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(REGS)); }
 template <int REGS> __device__ __forceinline__ void reg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(REGS)); }
 
-__device__ __forceinline__ int entry_state(int entry, int w) { return (entry >> (LVSA_ITEM_J_BITS + 2 * w)) & 3; }
+template <int V> struct StaticInt { __device__ constexpr operator int() const { return V; } };
 
-template <int NS>
+__device__ __forceinline__ int entry_state(int entry, int w) { return (entry >> (LVSA_ITEM_J_BITS + 2 * w)) & 3; }
+// 32-column chunks of the kv tile that are computed: 4 for a 128-column tile, fewer for a narrow
+// frame-aligned tile (reading R25)
+__device__ __forceinline__ int entry_chunks(int entry) { return (int)((uint32_t)entry >> LVSA_ITEM_W_SHIFT) + 1; }
+
+// VARW = false: every kv tile is 128 columns from token j * 128 (LVSA_KV_TILES_TOKEN0); the list entry
+// alone describes it and the widths are compile-time constants.  VARW = true: frame-aligned kv tiles
+// (LVSA_KV_TILES_FRAME_ALIGNED, reading R25): the first token comes from item_col0[] and the width
+// (32 .. 128 columns) from the entry, in the producer, the issuer and the softmax warps.
+template <int NS, bool VARW>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1)
 lvsa_attn_sm100_pair_kernel(const __grid_constant__ CUtensorMap tmap_q,
                             const __grid_constant__ CUtensorMap tmap_k,   // box 64 rows
                             const __grid_constant__ CUtensorMap tmap_v,   // box 128 rows
                             __nv_bfloat16 *__restrict__ out, float *__restrict__ lse,
                             const int32_t *__restrict__ item_ptr, const int32_t *__restrict__ item_tiles,
+                            const int32_t *__restrict__ item_col0,
                             const uint32_t *__restrict__ a_bits, int words, long long N, int P, int T,
                             int H, int h0, int hc, int n_items, long long n_work, long long sn, long long sh,
                             long long sb, float scale_log2) {
@@ -138,9 +145,7 @@ lvsa_attn_sm100_pair_kernel(const __grid_constant__ CUtensorMap tmap_q,
         const uint32_t pa_full0 = map_to_cta(bar(SM::PA_FULL), 0);           // the leader's barriers
         const uint32_t pb_full0 = map_to_cta(bar(SM::PB_FULL), 0);
         const uint32_t ofree = map_to_cta(bar(SM::O_FREE), 0);
-#ifndef LVSA_DIAG_NOSOFTMAX
         if (w == 1) tok_pass();     // the first token: tile 0 belongs to warpgroup 0
-#endif
         uint32_t tc = 0;            // kv tiles of this CTA so far (all items); tile tc belongs to warpgroup tc & 1
         uint32_t oc = 0;            // items finished
         for (long long work = pair; work < n_work; work += n_pairs) {
@@ -151,10 +156,18 @@ lvsa_attn_sm100_pair_kernel(const __grid_constant__ CUtensorMap tmap_q,
             const uint32_t *arow = a_bits + (size_t)fq * words;
             const int e0 = item_ptr[item], e1 = item_ptr[item + 1];
             float m_run = -INFINITY, l_run = 0.f;   // m_run: my copy of m_ref; l_run: my tiles' part of the row sum
-            for (int e = e0 + (int)((w - tc) & 1u); e < e1; e += 2) {
+            // the list entries are fetched one tile ahead so that the load never sits in front of a decision
+            const int e_first = e0 + (int)((w - tc) & 1u);
+            int entry_nx = e_first < e1 ? __ldg(item_tiles + e_first) : 0;
+            int col0_nx = (VARW && e_first < e1) ? __ldg(item_col0 + e_first) : 0;
+            for (int e = e_first; e < e1; e += 2) {
                 const uint32_t t_me = tc + (uint32_t)(e - e0);               // running index of this tile
-                const int entry = __ldg(item_tiles + e);
+                const int entry = entry_nx;
+                // first token of the kv tile (PARTIAL tiles need it) and its 32-column chunks
+                const int tile_col0 = VARW ? col0_nx : (entry & LVSA_ITEM_J_MASK) * BT;
+                if (e + 2 < e1) { entry_nx = __ldg(item_tiles + e + 2); if (VARW) col0_nx = __ldg(item_col0 + e + 2); }
                 const int st = entry_state(entry, (int)rank);
+                const int nch = VARW ? entry_chunks(entry) : 4;
                 const bool first = (e == e0);
 
                 // three S/P buffers in rotation: S(t+2) is computed while the softmax of tile t runs, and is
@@ -164,12 +177,6 @@ lvsa_attn_sm100_pair_kernel(const __grid_constant__ CUtensorMap tmap_q,
                 const uint32_t pa_full = pa_full0 + 8u * buf, pb_full = pb_full0 + 8u * buf;
                 mbar_wait(bar(SM::S_FULL + buf), (t_me / 3u) & 1u);
                 tc_fence_after();
-#ifdef LVSA_DIAG_NOSOFTMAX   // timing diagnostic only (wrong results): MMA/TMA pipeline alone
-                tc_fence_before(); __syncwarp();
-                if (lane == 0) { mbar_arrive_cluster(pa_full); mbar_arrive_cluster(pb_full); }
-                l_run = 1.f; m_run = 0.f;
-                continue;
-#endif
                 if (st == LVSA_ST_SKIP) {
                     // the pair's MMAs cover both q tiles for every listed kv tile; a tile that is not in
                     // MY q tile's list contributes nothing: P = 0.  The token still moves on.
@@ -187,109 +194,132 @@ lvsa_attn_sm100_pair_kernel(const __grid_constant__ CUtensorMap tmap_q,
                     if (lane == 0) { mbar_arrive_cluster(pa_full); mbar_arrive_cluster(pb_full); }
                     continue;
                 }
-                float s[BT];
+                // The body below is instantiated twice: with the chunk count as a compile-time 4 (a
+                // 128-column tile: no per-chunk tests, the four TMEM loads issue back to back) and with
+                // the run-time count of a narrow frame-aligned tile.
+                auto tile_body = [&](auto nch_) {
+                    const int nchv = nch_;
+                    float s[BT];
 #pragma unroll
-                for (int c = 0; c < 4; ++c) {
-                    uint32_t r[32];
-                    tmem_ld_32x32b_x32(tS + c * 32, r);
+                    for (int c = 0; c < 4; ++c) {
+                        if (c < nchv) {          // warp-uniform
+                            uint32_t r[32];
+                            tmem_ld_32x32b_x32(tS + c * 32, r);
 #pragma unroll
-                    for (int x = 0; x < 32; ++x) s[c * 32 + x] = __uint_as_float(r[x]);
-                }
-                tmem_wait_ld();
-
-                uint32_t cm[4] = {~0u, ~0u, ~0u, ~0u};   // columns of this tile my row may attend to
-                if (st == LVSA_ST_PARTIAL) {
-                    cm[0] = cm[1] = cm[2] = cm[3] = 0u;
-                    const long long col0 = (long long)(entry & LVSA_ITEM_J_MASK) * BT;
-                    const long long cend = min(col0 + BT, N);
-                    int g = min((int)(col0 / P), T - 1);
-                    for (long long fs = (long long)g * P, fe; fs < cend; fs = fe, ++g) {
-                        fe = (g == T - 1) ? N : fs + P;
-                        if ((arow[g >> 5] >> (g & 31)) & 1u) {
-                            const int lo = (int)(max(fs, col0) - col0), hi = (int)(min(fe, cend) - col0);
+                            for (int x = 0; x < 32; ++x) s[c * 32 + x] = __uint_as_float(r[x]);
+                        } else {                // columns a narrow tile does not have
 #pragma unroll
-                            for (int x = 0; x < 4; ++x) cm[x] |= range_mask32(lo, hi, x);
+                            for (int x = 0; x < 32; ++x) s[c * 32 + x] = -INFINITY;
                         }
                     }
+                    tmem_wait_ld();
+
+                    uint32_t cm[4] = {~0u, ~0u, ~0u, ~0u};   // columns of this tile my row may attend to
+                    if (st == LVSA_ST_PARTIAL) {
+                        cm[0] = cm[1] = cm[2] = cm[3] = 0u;
+                        const long long col0 = tile_col0;
+                        int g = min((int)((unsigned)tile_col0 / (unsigned)P), T - 1);
+                        // token-0 tiles: the columns run to the end of the tile (or N) across frame boundaries;
+                        // frame-aligned tiles: they stop at the end of the tile's frame (the rest is padding)
+                        const long long lim = !VARW ? N : (g == T - 1 ? N : (long long)(g + 1) * P);
+                        const long long cend = min(col0 + 32 * nchv, lim);
+                        for (long long fs = (long long)g * P, fe; fs < cend; fs = fe, ++g) {
+                            fe = (g == T - 1) ? N : fs + P;
+                            if ((arow[g >> 5] >> (g & 31)) & 1u) {
+                                const int lo = (int)(max(fs, col0) - col0), hi = (int)(min(fe, cend) - col0);
 #pragma unroll
-                    for (int c = 0; c < BT; ++c)
-                        if (!((cm[c >> 5] >> (c & 31)) & 1u)) s[c] = -INFINITY;
-                }
-                const float rm = lvsa_sm::row_max<BT>(s) * scale_log2;
+                                for (int x = 0; x < 4; ++x) cm[x] |= range_mask32(lo, hi, x);
+                            }
+                        }
+#pragma unroll
+                        for (int c = 0; c < BT; ++c)
+                            if (!((cm[c >> 5] >> (c & 31)) & 1u)) s[c] = -INFINITY;
+                    }
+                    const float rm = lvsa_sm::row_max<BT>(s) * scale_log2;
 
-                // ---- ordered phase: read the shared reference, decide, write it back
-                tok_wait();
-                bool grow;
-                float m_new;
-                if (first) {
-                    grow = false; m_new = rm; m_run = rm;          // the first tile of the item sets the reference
-                } else {
-                    const float m_sh = *m_ref;                      // may have been raised by the other warpgroup
-                    if (m_sh != m_run) { l_run *= fast_exp2(m_run - m_sh); m_run = m_sh; }   // exp2(-inf - x) = 0, l_run = 0 then
-                    grow = rm > m_run + RESCALE_THRESHOLD;
-                    m_new = grow ? rm : m_run;
-                }
-                *m_ref = m_new;
-                tok_pass();
-                // ---- end of the ordered phase
+                    // ---- ordered phase: read the shared reference, decide, write it back
+                    tok_wait();
+                    bool grow;
+                    float m_new;
+                    if (first) {
+                        grow = false; m_new = rm; m_run = rm;          // the first tile of the item sets the reference
+                    } else {
+                        const float m_sh = *m_ref;                      // may have been raised by the other warpgroup
+                        if (m_sh != m_run) { l_run *= fast_exp2(m_run - m_sh); m_run = m_sh; }   // exp2(-inf - x) = 0, l_run = 0 then
+                        grow = rm > m_run + RESCALE_THRESHOLD;
+                        m_new = grow ? rm : m_run;
+                    }
+                    *m_ref = m_new;
+                    tok_pass();
+                    // ---- end of the ordered phase
 
-                if (__any_sync(0xffffffffu, grow)) {
-                    // O is rescaled in place once every PV issued so far has landed (the other
-                    // warpgroup's tile t_me - 1 included).  PV(t) commits to PV_DONE[t & 1].  S_FULL of this
-                    // tile implies PV(t_me - 3) completed, the previous phase of that barrier, so the
-                    // parity wait is unambiguous.  PV(t_me) cannot be issued before this warpgroup
-                    // publishes P below.
-                    mbar_wait(bar(SM::PV_DONE + ((t_me - 1u) & 1u)), ((t_me - 1u) >> 1) & 1u);
-                    tc_fence_after();
-                    const float corr = grow ? fast_exp2(m_run - m_new) : 1.f;
-                    if (grow) { l_run *= corr; m_run = m_new; }
+                    if (__any_sync(0xffffffffu, grow)) {
+                        // O is rescaled in place once every PV issued so far has landed (the other
+                        // warpgroup's tile t_me - 1 included).  PV(t) commits to PV_DONE[t & 1].  S_FULL of this
+                        // tile implies PV(t_me - 3) completed, the previous phase of that barrier, so the
+                        // parity wait is unambiguous.  PV(t_me) cannot be issued before this warpgroup
+                        // publishes P below.
+                        mbar_wait(bar(SM::PV_DONE + ((t_me - 1u) & 1u)), ((t_me - 1u) >> 1) & 1u);
+                        tc_fence_after();
+                        const float corr = grow ? fast_exp2(m_run - m_new) : 1.f;
+                        if (grow) { l_run *= corr; m_run = m_new; }
 #pragma unroll 1
-                    for (int c = 0; c < 8; ++c) {
-                        uint32_t r[16];
-                        tmem_ld_32x32b_x16(tO + c * 16, r);
-                        tmem_wait_ld();
+                        for (int c = 0; c < 8; ++c) {
+                            uint32_t r[16];
+                            tmem_ld_32x32b_x16(tO + c * 16, r);
+                            tmem_wait_ld();
 #pragma unroll
-                        for (int x = 0; x < 16; ++x) r[x] = __float_as_uint(__uint_as_float(r[x]) * corr);
-                        tmem_st_32x32b_x16(tO + c * 16, r);
-                    }
-                }
-                const float m_use = (m_run == -INFINITY) ? 0.f : m_run;
-                const uint64_t negm2 = lvsa_sm::pack2(-m_use, -m_use);
-                uint64_t lsum = lvsa_sm::pack2(0.f, 0.f);
-                auto publish = [&](uint32_t which) {
-                    tmem_wait_st();
-                    tc_fence_before();
-                    __syncwarp();
-                    if (lane == 0) mbar_arrive_cluster(which);
-                };
-                if (st == LVSA_ST_FULL) {
-#pragma unroll
-                    for (int c = 0; c < 4; ++c) {
-                        uint32_t pk[16];
-                        lvsa_sm::exp_chunk32<LVSA_POLY_PAIRS>(s, c * 32, scale2, negm2, pk, lsum);
-                        tmem_st_32x32b_x16(tS + c * 16, pk);
-                        if (c == 1) publish(pa_full);
-                    }
-                } else {   // masked logits are -inf: the MUFU path gives exact zeros
-#pragma unroll
-                    for (int c = 0; c < 4; ++c) {
-                        uint32_t pk[16];
-                        if (cm[c] == 0u) {   // a fully masked group of 32 columns: P = 0 without the exponentials
-#pragma unroll
-                            for (int x = 0; x < 16; ++x) pk[x] = 0u;
-                        } else {
-                            lvsa_sm::exp_chunk32<0>(s, c * 32, scale2, negm2, pk, lsum);
+                            for (int x = 0; x < 16; ++x) r[x] = __float_as_uint(__uint_as_float(r[x]) * corr);
+                            tmem_st_32x32b_x16(tO + c * 16, r);
                         }
-                        tmem_st_32x32b_x16(tS + c * 16, pk);
-                        if (c == 1) publish(pa_full);
                     }
-                }
-                publish(pb_full);
-                {
-                    float la, lb;
-                    lvsa_sm::unpack2(lsum, la, lb);
-                    l_run += la + lb;
-                }
+                    const float m_use = (m_run == -INFINITY) ? 0.f : m_run;
+                    const uint64_t negm2 = lvsa_sm::pack2(-m_use, -m_use);
+                    uint64_t lsum = lvsa_sm::pack2(0.f, 0.f);
+                    auto publish = [&](uint32_t which) {
+                        tmem_wait_st();
+                        tc_fence_before();
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive_cluster(which);
+                    };
+                    // P for the nch chunks of the tile; the first half of P (or all of a narrow tile) is
+                    // published as soon as it is in TMEM so that the PV MMAs can start.  Masked logits are
+                    // -inf: the MUFU gives exact zeros; a fully masked chunk skips the exponentials.
+                    const int pa_at = min(1, nchv - 1);
+                    if (st == LVSA_ST_FULL) {
+#pragma unroll
+                        for (int c = 0; c < 4; ++c) {
+                            if (c < nchv) {
+                                uint32_t pk[16];
+                                lvsa_sm::exp_chunk32(s, c * 32, scale2, negm2, pk, lsum);
+                                tmem_st_32x32b_x16(tS + c * 16, pk);
+                                if (c == pa_at) publish(pa_full);
+                            }
+                        }
+                    } else
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) {
+                        if (c < nchv) {
+                            uint32_t pk[16];
+                            if (cm[c] == 0u) {
+#pragma unroll
+                                for (int x = 0; x < 16; ++x) pk[x] = 0u;
+                            } else {
+                                lvsa_sm::exp_chunk32(s, c * 32, scale2, negm2, pk, lsum);
+                            }
+                            tmem_st_32x32b_x16(tS + c * 16, pk);
+                            if (c == pa_at) publish(pa_full);
+                        }
+                    }
+                    publish(pb_full);
+                    {
+                        float la, lb;
+                        lvsa_sm::unpack2(lsum, la, lb);
+                        l_run += la + lb;
+                    }
+                };
+                if (!VARW || nch == 4) tile_body(StaticInt<4>{});
+                else tile_body(nch);
             }
             tc += (uint32_t)(e1 - e0);
             if (e0 < e1) {
@@ -330,9 +360,7 @@ lvsa_attn_sm100_pair_kernel(const __grid_constant__ CUtensorMap tmap_q,
             }
         }
         // drain the token that is left on one of the two barriers
-#ifndef LVSA_DIAG_NOSOFTMAX
         if ((tc & 1u) == (uint32_t)w) tok_wait();
-#endif
     } else {
         reg_dec<88>();
         if (warp == 8 && lane == 0) {
@@ -342,15 +370,20 @@ lvsa_attn_sm100_pair_kernel(const __grid_constant__ CUtensorMap tmap_q,
             // issuer consumes: K(0), K(1), then per tile j: K(j+2), V(j).
             const uint32_t q_full_L = map_to_cta(bar(SM::Q_FULL), 0);
             uint32_t kv_it = 0, qi = 0;
-            auto push = [&](const CUtensorMap *tm, bool is_k, int col0, int h, int b) {
+            // col0 = first token of the kv tile; nt = its computed columns.  K: CTA r supplies columns
+            // [r nt/2, (r+1) nt/2) of S, i.e. kv rows col0 + r nt/2 ... (the 64-row box over-reads for a
+            // narrow tile; the MMA uses the first nt/2 rows).  V: all rows of the tile, my 64 channels.
+            auto push = [&](const CUtensorMap *tm, bool is_k, int e, int h, int b) {
+                const int col0 = VARW ? __ldg(item_col0 + e) : (__ldg(item_tiles + e) & LVSA_ITEM_J_MASK) * BT;
+                const int nt = VARW ? 32 * entry_chunks(__ldg(item_tiles + e)) : BT;
                 const uint32_t stage = kv_it % NS, n = kv_it / NS;
                 mbar_wait(bar(SM::KV_EMPTY + stage), (n & 1u) ^ 1u);
                 if (rank == 0) mbar_expect_tx(bar(SM::KV_FULL + stage), 2 * STAGE_BYTES);
                 const uint32_t dst = sRing + stage * STAGE_BYTES;
                 const uint32_t full_L = map_to_cta(bar(SM::KV_FULL + stage), 0);
                 if (is_k) {   // kv rows [col0 + 64 rank, +64), channels [0,64) and [64,128): two 8 KB spans
-                    tma_load_4d_pair(dst, tm, full_L, 0, h, col0 + 64 * (int)rank, b);
-                    tma_load_4d_pair(dst + 8192, tm, full_L, 64, h, col0 + 64 * (int)rank, b);
+                    tma_load_4d_pair(dst, tm, full_L, 0, h, col0 + (nt / 2) * (int)rank, b);
+                    tma_load_4d_pair(dst + 8192, tm, full_L, 64, h, col0 + (nt / 2) * (int)rank, b);
                 } else {      // channels [64 rank, +64) of all 128 kv rows: one 16 KB span
                     tma_load_4d_pair(dst, tm, full_L, 64 * (int)rank, h, col0, b);
                 }
@@ -367,23 +400,26 @@ lvsa_attn_sm100_pair_kernel(const __grid_constant__ CUtensorMap tmap_q,
                 tma_load_4d_pair(sQ, &tmap_q, q_full_L, 0, h, (int)row0, b);
                 tma_load_4d_pair(sQ + SPAN_BYTES, &tmap_q, q_full_L, 64, h, (int)row0, b);
                 ++qi;
-                if (e0 < e1) push(&tmap_k, true, (__ldg(item_tiles + e0) & LVSA_ITEM_J_MASK) * BT, h, b);
-                if (e0 + 1 < e1) push(&tmap_k, true, (__ldg(item_tiles + e0 + 1) & LVSA_ITEM_J_MASK) * BT, h, b);
+                if (e0 < e1) push(&tmap_k, true, e0, h, b);
+                if (e0 + 1 < e1) push(&tmap_k, true, e0 + 1, h, b);
                 for (int e = e0; e < e1; ++e) {
-                    if (e + 2 < e1) push(&tmap_k, true, (__ldg(item_tiles + e + 2) & LVSA_ITEM_J_MASK) * BT, h, b);
-                    push(&tmap_v, false, (__ldg(item_tiles + e) & LVSA_ITEM_J_MASK) * BT, h, b);
+                    if (e + 2 < e1) push(&tmap_k, true, e + 2, h, b);
+                    push(&tmap_v, false, e, h, b);
                 }
             }
         } else if (warp == 9 && rank == 0) {
             // =========================================================== MMA issuer (leader CTA)
-            constexpr uint32_t IDESC_S = umma_idesc_bf16(256, BT, 0);
+            constexpr uint32_t IDESC_S0 = umma_idesc_bf16(256, 0, 0);   // N is filled in per tile
             constexpr uint32_t IDESC_O = umma_idesc_bf16(256, D, 1);
             const uint64_t dQ = umma_smem_desc_sw128(sQ, 16);
             const uint64_t dRing = umma_smem_desc_sw128(sRing, 16);
             const uint32_t tO = tmem_base + 384;
             // S(buf) = Q K^T: A = Q (128 rows per CTA, two 16 KB spans), B = my/peer K half (64 rows
             // per CTA, two 8 KB spans); 8 k-blocks of 16 channels
-            auto issue_S = [&](uint32_t buf, uint32_t stage, bool last_of_item) {
+            auto issue_S = [&](uint32_t buf, uint32_t stage, bool last_of_item, int nt) {
+                // a full tile takes the compile-time descriptor (N = 128), a narrow one builds its own
+                constexpr uint32_t IDESC_S128 = IDESC_S0 | ((uint32_t)(BT >> 3) << 17);
+                const uint32_t IDESC_S = nt == BT ? IDESC_S128 : (IDESC_S0 | ((uint32_t)(nt >> 3) << 17));
 #pragma unroll
                 for (int kk = 0; kk < 8; ++kk) {
                     const uint32_t offA = (uint32_t)((kk >> 2) * SPAN_BYTES + (kk & 3) * 32) >> 4;
@@ -397,13 +433,28 @@ lvsa_attn_sm100_pair_kernel(const __grid_constant__ CUtensorMap tmap_q,
             };
             // O += P(buf) V: A = P from TMEM (2 bf16 per column), B = V half (MN-major, 64 channels per
             // CTA = one 128 B span; 16 kv rows = 2048 B per k-block)
-            auto issue_PV = [&](uint32_t buf, uint32_t stage, bool accumulate, int half) {
+            // nt / 16 k-blocks of 16 kv rows; half 0 = blocks 0..3, half 1 = blocks 4..7 (as far as the tile has them)
+            auto issue_PV = [&](uint32_t buf, uint32_t stage, bool accumulate, int half, int nt) {
+                if (nt == BT) {
 #pragma unroll
-                for (int kk = 4 * half; kk < 4 * half + 4; ++kk)
-                    umma_ts_pair(tO, tmem_base + buf * 128 + kk * 8,
-                                 dRing + (uint64_t)((stage * STAGE_BYTES + (uint32_t)kk * 2048u) >> 4), IDESC_O,
-                                 (accumulate || kk > 0) ? 1u : 0u);
+                    for (int kk = 4 * half; kk < 4 * half + 4; ++kk)
+                        umma_ts_pair(tO, tmem_base + buf * 128 + kk * 8,
+                                     dRing + (uint64_t)((stage * STAGE_BYTES + (uint32_t)kk * 2048u) >> 4), IDESC_O,
+                                     (accumulate || kk > 0) ? 1u : 0u);
+                } else {
+#pragma unroll
+                    for (int kk = 4 * half; kk < 4 * half + 4; ++kk)
+                        if (kk * 16 < nt)
+                            umma_ts_pair(tO, tmem_base + buf * 128 + kk * 8,
+                                         dRing + (uint64_t)((stage * STAGE_BYTES + (uint32_t)kk * 2048u) >> 4), IDESC_O,
+                                         (accumulate || kk > 0) ? 1u : 0u);
+                }
             };
+            // the width is made warp-uniform explicitly (shuffle from lane 0): it feeds the instruction
+            // descriptor, which lives in a uniform register, and a value the compiler cannot prove uniform
+            // costs a per-instruction waterfall loop
+            auto uniform_nt = [&](int raw_entry) { return __shfl_sync(0xffffffffu, 32 * entry_chunks(raw_entry), 0); };
+            auto tile_nt = [&](int e) { return VARW ? uniform_nt(__ldg(item_tiles + e)) : BT; };
             uint32_t kv_it = 0, qi = 0, tc = 0, oc = 0;
             auto next_stage = [&](uint32_t &stage) {
                 stage = kv_it % NS;
@@ -419,20 +470,28 @@ lvsa_attn_sm100_pair_kernel(const __grid_constant__ CUtensorMap tmap_q,
                 mbar_wait(bar(SM::Q_FULL), qi & 1u); ++qi;
                 // S of the first two tiles; the buffer of tile t is t % 3 (running count), its previous
                 // P (tile t - 3) was read by a PV issued earlier
+                // widths of tiles j, j+1, j+2 (nt0, nt1, nt2); the entry of tile j+3 is fetched one
+                // iteration before it is needed, so no load sits in front of an MMA issue
+                int nt0 = n > 0 ? tile_nt(e0) : 0, nt1 = n > 1 ? tile_nt(e0 + 1) : 0, nt2 = n > 2 ? tile_nt(e0 + 2) : 0;
                 for (int j = 0; j < 2 && j < n; ++j) {
                     uint32_t stage;
                     next_stage(stage);
                     tc_fence_after();
-                    if (elect_one_sync()) issue_S((tc + j) % 3u, stage, j == n - 1);
+                    const int nt = j == 0 ? nt0 : nt1;
+                    if (elect_one_sync()) issue_S((tc + j) % 3u, stage, j == n - 1, nt);
                     __syncwarp();
                 }
                 for (int j = 0; j < n; ++j, ++tc) {
                     const uint32_t buf = tc % 3u, par = (tc / 3u) & 1u;
+                    const int nt_pv = nt0;
+                    // entry of tile j + 3: loaded now, shuffled (which waits for the load) at the end of the iteration
+                    const int raw3 = (VARW && j + 3 < n) ? __ldg(item_tiles + e0 + j + 3) : 0;
                     if (j + 2 < n) {
+                        const int nt = nt2;
                         uint32_t stage;
                         next_stage(stage);
                         tc_fence_after();
-                        if (elect_one_sync()) issue_S((tc + 2u) % 3u, stage, j + 2 == n - 1);   // after PV(tc-1): its buffer is free
+                        if (elect_one_sync()) issue_S((tc + 2u) % 3u, stage, j + 2 == n - 1, nt);   // after PV(tc-1): its buffer is free
                         __syncwarp();
                     }
                     uint32_t stageV;
@@ -440,16 +499,17 @@ lvsa_attn_sm100_pair_kernel(const __grid_constant__ CUtensorMap tmap_q,
                     if (j == 0) mbar_wait(bar(SM::O_FREE), (oc & 1u) ^ 1u);
                     mbar_wait(bar(SM::PA_FULL + buf), par);
                     tc_fence_after();
-                    if (elect_one_sync()) issue_PV(buf, stageV, j > 0, 0);
+                    if (elect_one_sync()) issue_PV(buf, stageV, j > 0, 0, nt_pv);
                     __syncwarp();
                     mbar_wait(bar(SM::PB_FULL + buf), par);
                     tc_fence_after();
                     if (elect_one_sync()) {
-                        issue_PV(buf, stageV, j > 0, 1);
+                        issue_PV(buf, stageV, j > 0, 1, nt_pv);
                         umma_commit_pair(bar(SM::PV_DONE + (tc & 1u)));
                         umma_commit_pair(bar(SM::KV_EMPTY + stageV));
                     }
                     __syncwarp();
+                    nt0 = nt1; nt1 = nt2; nt2 = VARW ? uniform_nt(raw3) : BT;
                 }
                 if (n > 0) {
                     if (elect_one_sync()) umma_commit_pair(bar(SM::O_FULL));
@@ -479,7 +539,9 @@ lvsa_status_t lvsa_attn_sm100_pair_prepare(int device) {
     if (device < 0 || device >= LVSA_MAX_DEVICES) { lvsa_set_error("device ordinal out of range"); return LVSA_EUNSUPPORTED; }
     if (g_pair_n_sm[device] != 0) return LVSA_OK;
     using SM = SmemP<LVSA_PAIR_STAGES>;
-    LVSA_CUDA_TRY(cudaFuncSetAttribute(lvsa_attn_sm100_pair_kernel<LVSA_PAIR_STAGES>,
+    LVSA_CUDA_TRY(cudaFuncSetAttribute(lvsa_attn_sm100_pair_kernel<LVSA_PAIR_STAGES, false>,
+                                       cudaFuncAttributeMaxDynamicSharedMemorySize, SM::BYTES));
+    LVSA_CUDA_TRY(cudaFuncSetAttribute(lvsa_attn_sm100_pair_kernel<LVSA_PAIR_STAGES, true>,
                                        cudaFuncAttributeMaxDynamicSharedMemorySize, SM::BYTES));
     int n = 0;
     LVSA_CUDA_TRY(cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, device));
@@ -504,8 +566,10 @@ lvsa_status_t lvsa_attn_sm100_pair_launch_heads(const lvsa_index *ix, const void
     const lvsa_strides sd = lvsa_layout_strides(ix);
     if (n_work < n_pairs) n_pairs = n_work;
     const float scale_log2 = ix->p.softmax_scale * 1.4426950408889634f;
-    lvsa_attn_sm100_pair_kernel<NS><<<(unsigned)(2 * n_pairs), NTHREADS, SM::BYTES, stream>>>(
-        mq, mk, mv, (__nv_bfloat16 *)out, lse, ix->d_item_ptr, ix->d_item_tiles, ix->d_abits, ix->words,
+    auto kern = ix->p.kv_tiling == LVSA_KV_TILES_FRAME_ALIGNED ? lvsa_attn_sm100_pair_kernel<NS, true>
+                                                               : lvsa_attn_sm100_pair_kernel<NS, false>;
+    kern<<<(unsigned)(2 * n_pairs), NTHREADS, SM::BYTES, stream>>>(
+        mq, mk, mv, (__nv_bfloat16 *)out, lse, ix->d_item_ptr, ix->d_item_tiles, ix->d_item_col0, ix->d_abits, ix->words,
         (long long)ix->N, ix->p.P, ix->Tf, ix->p.H, h0, hc, (int)ix->n_items, n_work, sd.n, sd.h, sd.b, scale_log2);
     LVSA_CUDA_TRY(cudaGetLastError());
     return LVSA_OK;

@@ -93,6 +93,7 @@ lvsa_status_t lvsa_build_block_index_ex(const lvsa_params_t *params, void *strea
     if (p.kernel < LVSA_KERNEL_AUTO || p.kernel > LVSA_KERNEL_TCGEN05_V0) { lvsa_set_error("bad kernel"); return LVSA_EINVAL; }
     if (p.layout != LVSA_LAYOUT_NHD && p.layout != LVSA_LAYOUT_HND) { lvsa_set_error("bad layout"); return LVSA_EINVAL; }
     if (p.host_groups < 0) { lvsa_set_error("host_groups must be >= 0"); return LVSA_EINVAL; }
+    if (p.kv_tiling != LVSA_KV_TILES_TOKEN0 && p.kv_tiling != LVSA_KV_TILES_FRAME_ALIGNED) { lvsa_set_error("bad kv_tiling"); return LVSA_EINVAL; }
     if (p.T > 4096) { lvsa_set_error("T > 4096 frames is not supported"); return LVSA_EUNSUPPORTED; }
     if (p.d != 64 && p.d != 128) { lvsa_set_error("head dim must be 64 or 128"); return LVSA_EUNSUPPORTED; }
     if (p.tile_q == 0) p.tile_q = p.d;
@@ -114,6 +115,11 @@ lvsa_status_t lvsa_build_block_index_ex(const lvsa_params_t *params, void *strea
     ix->Tf = p.T + (p.n_text > 0 ? 1 : 0);
     ix->nq = (int32_t)((ix->N + p.tile_q - 1) / p.tile_q);
     ix->nk = (int32_t)((ix->N + p.tile_k - 1) / p.tile_k);
+    if (p.kv_tiling == LVSA_KV_TILES_FRAME_ALIGNED) {   // ceil(P/Bk) tiles per frame + the text tiles (R25)
+        const long long nk = (long long)p.T * lvsa_kv_tiles_per_frame(p.P, p.tile_k) + (p.n_text + p.tile_k - 1) / p.tile_k;
+        if (nk >= (1ll << LVSA_ITEM_J_BITS)) { delete ix; lvsa_set_error("too many kv tiles"); return LVSA_EUNSUPPORTED; }
+        ix->nk = (int32_t)nk;
+    }
     ix->words = (ix->Tf + 31) / 32;
     ix->group = 2;
     if ((long long)ix->nq * ix->nk >= (1ll << 31)) {
@@ -126,6 +132,11 @@ lvsa_status_t lvsa_build_block_index_ex(const lvsa_params_t *params, void *strea
     if (ix->device < 0 || ix->device >= LVSA_MAX_DEVICES) { lvsa_index_destroy(ix); lvsa_set_error("device ordinal out of range"); return LVSA_EUNSUPPORTED; }
     lvsa_status_t st = lvsa_index_build_device(ix, (cudaStream_t)stream);
     if (st != LVSA_OK) { lvsa_index_destroy(ix); return st; }
+    if (use_tcgen05(ix) && p.kv_tiling == LVSA_KV_TILES_FRAME_ALIGNED && !lvsa_attn_uses_pair_kernel(ix)) {
+        lvsa_index_destroy(ix);
+        lvsa_set_error("frame-aligned kv tiles: CTA-pair kernel (d = 128) or SIMT kernel only");
+        return LVSA_EUNSUPPORTED;
+    }
     if (use_tcgen05(ix) && !lvsa_attn_sm100_supported(ix)) {
         lvsa_index_destroy(ix);
         lvsa_set_error("tcgen05 kernel: device is not sm_100 or shape unsupported");
@@ -325,7 +336,8 @@ lvsa_status_t lvsa_index_info(const lvsa_index_t *ix, lvsa_index_info_t *info) {
     info->tile_q = p.tile_q; info->tile_k = p.tile_k; info->nq = ix->nq; info->nk = ix->nk;
     info->T_per = ix->T_per; info->phase = ix->phase; info->n_global = ix->n_global;
     info->words = ix->words; info->dtype = p.dtype; info->n_text = p.n_text;
-    info->initial_anchors = p.initial_anchors; info->layout = p.layout;
+    info->initial_anchors = p.initial_anchors; info->layout = p.layout; info->kv_tiling = p.kv_tiling;
+    info->kept_cols = ix->kept_cols;
     info->kernel = !use_tcgen05(ix) ? LVSA_KERNEL_SIMT
                  : (p.kernel == LVSA_KERNEL_TCGEN05_V0 ? LVSA_KERNEL_TCGEN05_V0 : LVSA_KERNEL_TCGEN05);
     info->N = ix->N; info->nnz = ix->nnz; info->n_partial = ix->n_partial;
@@ -345,6 +357,17 @@ lvsa_status_t lvsa_index_copy_host(const lvsa_index_t *ix, int32_t *indptr, int3
     if (w_lo) LVSA_CUDA_TRY(cudaMemcpy(w_lo, ix->d_wlo, sizeof(int32_t) * T, cudaMemcpyDeviceToHost));
     if (w_hi) LVSA_CUDA_TRY(cudaMemcpy(w_hi, ix->d_whi, sizeof(int32_t) * T, cudaMemcpyDeviceToHost));
     if (a_bits) LVSA_CUDA_TRY(cudaMemcpy(a_bits, ix->d_abits, sizeof(uint32_t) * (size_t)ix->Tf * ix->words, cudaMemcpyDeviceToHost));
+    return LVSA_OK;
+}
+
+lvsa_status_t lvsa_index_copy_kv_tiles(const lvsa_index_t *ix, int32_t *col0, int32_t *width) {
+    if (ix == nullptr) { lvsa_set_error("NULL index"); return LVSA_EINVAL; }
+    const int aligned = ix->p.kv_tiling == LVSA_KV_TILES_FRAME_ALIGNED;
+    for (int j = 0; j < ix->nk; ++j) {
+        const lvsa_kv_tile t = lvsa_kv_tile_of(j, aligned, ix->p.tile_k, ix->p.P, ix->p.T, ix->N);
+        if (col0) col0[j] = (int32_t)t.c0;
+        if (width) width[j] = t.width;
+    }
     return LVSA_OK;
 }
 

@@ -98,13 +98,17 @@ __global__ void lvsa_frames_kernel(int T, int W, int a, int s, int tie_hi, int k
 // entry tagged with the per-q-tile state (skip / full / partial).
 //   FILL = false: counts[i] per q tile, icounts[g] per item.
 //   FILL = true : indices/flags at indptr[i] (the CSR), item_tiles at item_ptr[g].
-template <bool FILL>
-__global__ void lvsa_tiles_kernel(long long N, int P, int Tf, int Bq, int Bk, int nq, int nk, int words,
+//   ALIGNED = true: frame-aligned kv tiles (reading R25): tile j lies inside one frame, is PARTIAL
+//   iff some row of the q tile does not attend to that frame or its width is not a multiple of
+//   LVSA_KV_PAD; Tv = video frames (Tf minus the text pseudo-frame).
+template <bool FILL, bool ALIGNED>
+__global__ void lvsa_tiles_kernel(long long N, int P, int Tv, int Tf, int Bq, int Bk, int nq, int nk, int words,
                                   const uint32_t *__restrict__ a_bits,
                                   const int32_t *__restrict__ indptr, const int32_t *__restrict__ item_ptr,
                                   int32_t *__restrict__ counts, int32_t *__restrict__ icounts,
                                   int32_t *__restrict__ indices, uint8_t *__restrict__ flags,
-                                  int32_t *__restrict__ item_tiles, int32_t *__restrict__ meta) {
+                                  int32_t *__restrict__ item_tiles, int32_t *__restrict__ item_col0,
+                                  int32_t *__restrict__ meta, unsigned long long *__restrict__ kept_cols) {
     __shared__ int warp_tot[3][32];
     const int g = blockIdx.x, tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int nwarps = blockDim.x >> 5;
@@ -122,16 +126,28 @@ __global__ void lvsa_tiles_kernel(long long N, int P, int Tf, int Bq, int Bk, in
         fb[w] = (w == 0 || has1) ? min((int)(r1 / P), Tf - 1) : fa[w] - 1;   // empty range: no q tile 1
     }
     int run[3] = {0, 0, 0}, n_part = 0;
+    long long n_cols = 0;   // computed kv columns over the kept (q tile, kv tile) pairs of this thread
     int base[3] = {0, 0, 0};
     if (FILL) { base[0] = indptr[i0]; base[1] = has1 ? indptr[i1] : 0; base[2] = item_ptr[g]; }
     for (int j0 = 0; j0 < nk; j0 += blockDim.x) {
         const int j = j0 + tid;
         bool kept[2] = {false, false}, part[2] = {false, false};
+        long long c0 = 0;
+        int wpad = Bk;      // columns a kernel computes for this tile
         if (j < nk) {
-            const long long c0 = (long long)j * Bk;
-            const long long c1 = min(c0 + Bk, N) - 1;
-            const int g0 = min((int)(c0 / P), Tf - 1), g1 = min((int)(c1 / P), Tf - 1);
-            const bool tail = (c0 + Bk > N);  // columns >= N are never allowed
+            int g0, g1;
+            bool tail;
+            if (ALIGNED) {
+                const lvsa_kv_tile kt = lvsa_kv_tile_of(j, 1, Bk, P, Tv, N);
+                c0 = kt.c0; g0 = g1 = kt.g;
+                wpad = (kt.width + LVSA_KV_PAD - 1) / LVSA_KV_PAD * LVSA_KV_PAD;
+                tail = wpad != kt.width;          // padding columns are never allowed
+            } else {
+                c0 = (long long)j * Bk;
+                const long long c1 = min(c0 + Bk, N) - 1;
+                g0 = min((int)(c0 / P), Tf - 1); g1 = min((int)(c1 / P), Tf - 1);
+                tail = (c0 + Bk > N);             // columns >= N are never allowed
+            }
 #pragma unroll
             for (int w = 0; w < 2; ++w) {
                 part[w] = tail;
@@ -158,16 +174,22 @@ __global__ void lvsa_tiles_kernel(long long N, int P, int Tf, int Bq, int Bk, in
             if (kept[0]) {
                 const int pos = base[0] + run[0] + woff[0] + __popc(bal0 & below);
                 indices[pos] = j; flags[pos] = part[0] ? LVSA_TILE_PARTIAL : LVSA_TILE_FULL; n_part += part[0];
+                n_cols += wpad;
             }
             if (kept[1]) {
                 const int pos = base[1] + run[1] + woff[1] + __popc(bal1 & below);
                 indices[pos] = j; flags[pos] = part[1] ? LVSA_TILE_PARTIAL : LVSA_TILE_FULL; n_part += part[1];
+                n_cols += wpad;
             }
             if (kept[0] || kept[1]) {
                 const int st0 = kept[0] ? (part[0] ? LVSA_ST_PARTIAL : LVSA_ST_FULL) : LVSA_ST_SKIP;
                 const int st1 = kept[1] ? (part[1] ? LVSA_ST_PARTIAL : LVSA_ST_FULL) : LVSA_ST_SKIP;
-                item_tiles[base[2] + run[2] + woff[2] + __popc(balu & below)] =
-                    j | (st0 << LVSA_ITEM_J_BITS) | (st1 << (LVSA_ITEM_J_BITS + 2));
+                const int pos = base[2] + run[2] + woff[2] + __popc(balu & below);
+                // the width field has 2 bits: 32-column units (tiles wider than 128 do not exist)
+                const unsigned wbits = (unsigned)(min(wpad, 128) / 32 - 1);
+                item_tiles[pos] = (int32_t)((unsigned)j | ((unsigned)st0 << LVSA_ITEM_J_BITS) |
+                                            ((unsigned)st1 << (LVSA_ITEM_J_BITS + 2)) | (wbits << LVSA_ITEM_W_SHIFT));
+                item_col0[pos] = (int32_t)c0;
             }
         }
 #pragma unroll
@@ -178,6 +200,8 @@ __global__ void lvsa_tiles_kernel(long long N, int P, int Tf, int Bq, int Bk, in
     if (FILL) {
         n_part = __reduce_add_sync(0xffffffffu, n_part);
         if (lane == 0 && n_part) atomicAdd(&meta[1], n_part);
+        for (int o = 16; o > 0; o >>= 1) n_cols += __shfl_xor_sync(0xffffffffu, n_cols, o);
+        if (lane == 0 && n_cols) atomicAdd(kept_cols, (unsigned long long)n_cols);
     }
 }
 
@@ -272,9 +296,11 @@ lvsa_status_t lvsa_index_build_device(lvsa_index *ix, cudaStream_t stream) {
     const size_t o_flags = take((size_t)(ix->cap_nnz + 1));
     const size_t o_item_ptr = take(sizeof(int32_t) * ((size_t)ix->n_items + 1));
     const size_t o_item_tiles = take(sizeof(int32_t) * (size_t)(ix->cap_item_tiles + 1));
+    const size_t o_item_col0 = take(sizeof(int32_t) * (size_t)(ix->cap_item_tiles + 1));
+    const size_t o_kept_cols = take(sizeof(unsigned long long));
 
-    static bool pool_ready[64] = {};
-    if (ix->device >= 0 && ix->device < 64 && !pool_ready[ix->device]) {
+    static bool pool_ready[LVSA_MAX_DEVICES] = {};
+    if (!pool_ready[ix->device]) {
         cudaMemPool_t pool;
         LVSA_CUDA_TRY(cudaDeviceGetDefaultMemPool(&pool, ix->device));
         unsigned long long keep = ~0ull;   // keep freed arenas cached: rebuilds then allocate in microseconds
@@ -292,21 +318,28 @@ lvsa_status_t lvsa_index_build_device(lvsa_index *ix, cudaStream_t stream) {
     int32_t *d_counts = (int32_t *)(a + o_counts), *d_icounts = (int32_t *)(a + o_icounts);
     ix->d_indices = (int32_t *)(a + o_indices); ix->d_flags = a + o_flags;
     ix->d_item_ptr = (int32_t *)(a + o_item_ptr); ix->d_item_tiles = (int32_t *)(a + o_item_tiles);
+    ix->d_item_col0 = (int32_t *)(a + o_item_col0);
+    ix->d_kept_cols = (unsigned long long *)(a + o_kept_cols);
 
     LVSA_CUDA_TRY(cudaMemsetAsync(ix->d_meta, 0, sizeof(int32_t) * 8, stream));
+    LVSA_CUDA_TRY(cudaMemsetAsync(ix->d_kept_cols, 0, sizeof(unsigned long long), stream));
     lvsa_frames_kernel<<<1, 256, sizeof(uint32_t) * words, stream>>>(
         T, W, p.anchors, p.step, p.tie_break == LVSA_TIE_HI, p.initial_anchors, p.n_text > 0, words, ix->d_wlo, ix->d_whi,
         ix->d_abits, ix->d_meta);
     const int n_items = (int)ix->n_items;
-    lvsa_tiles_kernel<false><<<n_items, 256, 0, stream>>>(
-        (long long)ix->N, p.P, ix->Tf, p.tile_q, p.tile_k, ix->nq, ix->nk, words, ix->d_abits, nullptr, nullptr,
-        d_counts, d_icounts, nullptr, nullptr, nullptr, ix->d_meta);
+    const bool aligned = p.kv_tiling == LVSA_KV_TILES_FRAME_ALIGNED;
+    auto count_k = aligned ? lvsa_tiles_kernel<false, true> : lvsa_tiles_kernel<false, false>;
+    auto fill_k = aligned ? lvsa_tiles_kernel<true, true> : lvsa_tiles_kernel<true, false>;
+    count_k<<<n_items, 256, 0, stream>>>(
+        (long long)ix->N, p.P, T, ix->Tf, p.tile_q, p.tile_k, ix->nq, ix->nk, words, ix->d_abits, nullptr, nullptr,
+        d_counts, d_icounts, nullptr, nullptr, nullptr, nullptr, ix->d_meta, ix->d_kept_cols);
     lvsa_scan_kernel<<<2, 1024, 0, stream>>>(d_counts, ix->nq, ix->d_indptr, ix->d_meta + 0, (long long)ix->cap_nnz,
                                              d_icounts, n_items, ix->d_item_ptr, ix->d_meta + 2,
                                              (long long)ix->cap_item_tiles, ix->d_meta + 7);
-    lvsa_tiles_kernel<true><<<n_items, 256, 0, stream>>>(
-        (long long)ix->N, p.P, ix->Tf, p.tile_q, p.tile_k, ix->nq, ix->nk, words, ix->d_abits, ix->d_indptr,
-        ix->d_item_ptr, nullptr, nullptr, ix->d_indices, ix->d_flags, ix->d_item_tiles, ix->d_meta);
+    fill_k<<<n_items, 256, 0, stream>>>(
+        (long long)ix->N, p.P, T, ix->Tf, p.tile_q, p.tile_k, ix->nq, ix->nk, words, ix->d_abits, ix->d_indptr,
+        ix->d_item_ptr, nullptr, nullptr, ix->d_indices, ix->d_flags, ix->d_item_tiles, ix->d_item_col0, ix->d_meta,
+        ix->d_kept_cols);
     LVSA_CUDA_TRY(cudaGetLastError());
     ix->meta_fetched = false;
     return LVSA_OK;
@@ -317,7 +350,9 @@ lvsa_status_t lvsa_index_build_device(lvsa_index *ix, cudaStream_t stream) {
 lvsa_status_t lvsa_index_fetch_meta(const lvsa_index *ix) {
     if (ix->meta_fetched) return LVSA_OK;
     int32_t meta[8];
+    unsigned long long kept_cols = 0;
     LVSA_CUDA_TRY(cudaMemcpyAsync(meta, ix->d_meta, sizeof(meta), cudaMemcpyDeviceToHost, ix->build_stream));
+    LVSA_CUDA_TRY(cudaMemcpyAsync(&kept_cols, ix->d_kept_cols, sizeof(kept_cols), cudaMemcpyDeviceToHost, ix->build_stream));
     LVSA_CUDA_TRY(cudaStreamSynchronize(ix->build_stream));
     if (meta[7] != 0) {
         lvsa_set_error("internal: kept-tile count exceeds the allocation bound");
@@ -325,6 +360,7 @@ lvsa_status_t lvsa_index_fetch_meta(const lvsa_index *ix) {
     }
     ix->nnz = meta[0]; ix->n_partial = meta[1]; ix->n_item_tiles = meta[2];
     ix->T_per = meta[4]; ix->phase = meta[5]; ix->n_global = meta[6];
+    ix->kept_cols = (int64_t)kept_cols;
     ix->meta_fetched = true;
     return LVSA_OK;
 }

@@ -12,9 +12,41 @@
 // Work-item entry encoding for the attention kernels (one int32 per kv-tile visit of a q-tile
 // group).  bits [0,26): kv tile j.  bits [26,28): state for the group's q tile 0, bits [28,30):
 // state for q tile 1.  States:
+// bits [30,32): (computed columns of the kv tile) / 32 - 1, i.e. 3 for a 128-column tile, less for a
+// narrow frame-aligned tile (lvsa_params_t.kv_tiling).
 constexpr int LVSA_ST_SKIP = 0, LVSA_ST_FULL = 1, LVSA_ST_PARTIAL = 2;
 constexpr int LVSA_ITEM_J_BITS = 26;
 constexpr int LVSA_ITEM_J_MASK = (1 << LVSA_ITEM_J_BITS) - 1;
+constexpr int LVSA_ITEM_W_SHIFT = 30;
+
+// Geometry of kv tile j under either tiling (include/lvsa.h, readings R14 / R25): first token, valid
+// width, and the frame row of its first token.  T = video frames, Tf = T + (text pseudo-frame).
+struct lvsa_kv_tile { long long c0; int width; int g; };
+__host__ __device__ inline int lvsa_kv_tiles_per_frame(int P, int Bk) { return (P + Bk - 1) / Bk; }
+__host__ __device__ inline lvsa_kv_tile lvsa_kv_tile_of(int j, int frame_aligned, int Bk, int P, int T, long long N) {
+    lvsa_kv_tile t;
+    if (!frame_aligned) {
+        t.c0 = (long long)j * Bk;
+        t.width = (int)((t.c0 + Bk <= N) ? Bk : N - t.c0);
+        const long long f = t.c0 / P;
+        t.g = (int)(f < T ? f : T);
+        return t;
+    }
+    const int kpf = lvsa_kv_tiles_per_frame(P, Bk);
+    const int tau = j / kpf;
+    if (tau < T) {                      // video frame tau, tile k of it
+        const int k = j - tau * kpf;
+        t.c0 = (long long)tau * P + (long long)k * Bk;
+        t.width = (k + 1) * Bk <= P ? Bk : P - k * Bk;
+        t.g = tau;
+    } else {                            // text pseudo-frame (R23)
+        const int k = j - T * kpf;
+        t.c0 = (long long)T * P + (long long)k * Bk;
+        t.width = (int)((t.c0 + Bk <= N) ? Bk : N - t.c0);
+        t.g = T;
+    }
+    return t;
+}
 
 struct lvsa_index {
     lvsa_params_t p;  // with defaults resolved
@@ -47,6 +79,9 @@ struct lvsa_index {
     mutable int64_t n_item_tiles = 0;
     int32_t *d_item_ptr = nullptr;    // [n_items+1]
     int32_t *d_item_tiles = nullptr;  // [n_item_tiles], encoding above
+    int32_t *d_item_col0 = nullptr;   // [n_item_tiles], first token of the entry's kv tile
+    mutable int64_t kept_cols = 0;    // sum of computed kv columns over the kept pairs
+    unsigned long long *d_kept_cols = nullptr;
 };
 
 // Element strides of the token, head and batch axes of q, k, v, out (d is contiguous):

@@ -32,9 +32,11 @@ def test_header_constants_match_binding():
     src = open(os.path.join(ROOT, "include", "lvsa.h")).read()
     vals = {k: int(v) for k, v in re.findall(r"\b(LVSA_[A-Z0-9_]+)\s*=\s*(-?\d+)", src)}
     for name in ("KERNEL_AUTO", "KERNEL_SIMT", "KERNEL_TCGEN05", "KERNEL_TCGEN05_V0", "LAYOUT_NHD", "LAYOUT_HND",
+                 "KV_TILES_TOKEN0", "KV_TILES_FRAME_ALIGNED",
                  "DTYPE_BF16", "DTYPE_FP32", "TIE_LO", "TIE_HI", "TILE_FULL", "TILE_PARTIAL", "OK", "EINVAL",
                  "EUNSUPPORTED", "ECUDA", "ENOMEM"):
         assert vals["LVSA_" + name] == getattr(binding, name), name
+    assert int(re.search(r"#define LVSA_KV_PAD (\d+)", src).group(1)) == binding.KV_PAD
     # no debug hooks or environment switches in the product library
     csrc = os.path.join(ROOT, "paper_2605_31057_b200", "csrc")
     for f in os.listdir(csrc):
@@ -44,10 +46,10 @@ def test_header_constants_match_binding():
 
 
 def test_struct_sizes_match_header():
-    # 14 int32 + float + 4 int32; 22 int32 + 5 int64 (include/lvsa.h)
-    assert C.sizeof(binding.Params) == 19 * 4
-    assert C.sizeof(binding.IndexInfo) == 22 * 4 + 5 * 8
-    assert binding.IndexInfo.N.offset == 22 * 4
+    # 14 int32 + float + 5 int32; 24 int32 + 6 int64 (include/lvsa.h)
+    assert C.sizeof(binding.Params) == 20 * 4
+    assert C.sizeof(binding.IndexInfo) == 24 * 4 + 6 * 8
+    assert binding.IndexInfo.N.offset == 24 * 4
 
 
 def test_argument_validation_needs_no_gpu():
@@ -56,7 +58,8 @@ def test_argument_validation_needs_no_gpu():
            dict(T=4, P=4, H=1, d=64, layer=-1), dict(T=1 << 16, P=1 << 16, H=1, d=64),
            dict(T=4, P=4, H=1, d=64, tie_break=7), dict(T=4, P=4, H=1, d=64, initial_anchors=-1),
            dict(T=4, P=4, H=1, d=64, n_text=-1), dict(T=4, P=4, H=1, d=64, layout=2),
-           dict(T=4, P=4, H=1, d=64, kernel=4), dict(T=4, P=4, H=1, d=64, host_groups=-1)]
+           dict(T=4, P=4, H=1, d=64, kernel=4), dict(T=4, P=4, H=1, d=64, host_groups=-1),
+           dict(T=4, P=4, H=1, d=64, kv_tiling=2)]
     for kw in bad:
         with pytest.raises(binding.LvsaError) as ei:
             binding.lvsa_build_block_index_ex(**kw)
