@@ -217,23 +217,30 @@ lvsa_attn_sm100_pair_kernel(const __grid_constant__ CUtensorMap tmap_q,
                     uint32_t cm[4] = {~0u, ~0u, ~0u, ~0u};   // columns of this tile my row may attend to
                     if (st == LVSA_ST_PARTIAL) {
                         cm[0] = cm[1] = cm[2] = cm[3] = 0u;
-                        const long long col0 = tile_col0;
+                        // 32-bit arithmetic in coordinates relative to the tile's first token (N < 2^31)
+                        const int Ni = (int)N;
                         int g = min((int)((unsigned)tile_col0 / (unsigned)P), T - 1);
                         // token-0 tiles: the columns run to the end of the tile (or N) across frame boundaries;
                         // frame-aligned tiles: they stop at the end of the tile's frame (the rest is padding)
-                        const long long lim = !VARW ? N : (g == T - 1 ? N : (long long)(g + 1) * P);
-                        const long long cend = min(col0 + 32 * nchv, lim);
-                        for (long long fs = (long long)g * P, fe; fs < cend; fs = fe, ++g) {
-                            fe = (g == T - 1) ? N : fs + P;
+                        const int lim = (!VARW || g == T - 1) ? Ni - tile_col0 : (g + 1) * P - tile_col0;
+                        const int cend = min(32 * nchv, lim);
+                        for (int fs = g * P - tile_col0, fe; fs < cend; fs = fe, ++g) {
+                            fe = (g == T - 1) ? Ni - tile_col0 : fs + P;
                             if ((arow[g >> 5] >> (g & 31)) & 1u) {
-                                const int lo = (int)(max(fs, col0) - col0), hi = (int)(min(fe, cend) - col0);
+                                const int lo = max(fs, 0), hi = min(fe, cend);
 #pragma unroll
                                 for (int x = 0; x < 4; ++x) cm[x] |= range_mask32(lo, hi, x);
                             }
                         }
+                        // most rows of a PARTIAL tile are not masked at all (the flag is per q tile): a chunk
+                        // whose 32 columns are all allowed is left alone
 #pragma unroll
-                        for (int c = 0; c < BT; ++c)
-                            if (!((cm[c >> 5] >> (c & 31)) & 1u)) s[c] = -INFINITY;
+                        for (int c4 = 0; c4 < 4; ++c4)
+                            if (cm[c4] != ~0u) {
+#pragma unroll
+                                for (int x = 0; x < 32; ++x)
+                                    if (!((cm[c4] >> x) & 1u)) s[c4 * 32 + x] = -INFINITY;
+                            }
                     }
                     const float rm = lvsa_sm::row_max<BT>(s) * scale_log2;
 

@@ -56,6 +56,10 @@ WORKLOADS = {
                           steps=(25,), layers=(20,), n_layers=40),
     "hv1.5_2x": Workload("hv1.5_2x", 5, T=65, P=1590, H=16, d=128, tile=128, W=2, a=28,
                          steps=(0, 25, 49), layers=(27,), n_layers=54),
+    # the paper's second measured resolution, 720x1280 -> 45 x 80 latent tokens per frame, at the 6x
+    # horizon (Table 4); not a BASELINE.json config, same readings as wan1.3b_6x
+    "wan1.3b_6x_720p": Workload("wan1.3b_6x_720p", 3, T=121, P=3600, H=12, d=128, tile=128, W=2, a=16,
+                                steps=(25,), layers=(15,), n_layers=30),
     # non-contract variants used by the parity tests (ragged tiles, straddling frames)
     "tiny_straddle": Workload("tiny_straddle", 1, T=8, P=40, H=2, d=64, tile=64, W=1, a=2,
                               steps=tuple(range(10)), layers=(0,), n_layers=4),

@@ -159,6 +159,24 @@ def test_benched_variants_sampled_rows(name, window, anchors):
 
 
 @pytest.mark.slow
+def test_720p_shape_index_and_sampled_rows():
+    """The paper's other measured resolution (Table 4: 720 x 1280, 481 frames): N = 435 600,
+    nq * nk = 1.16e7, 1.34 GB per operand.  Index bit-exact, 1024 sampled rows against the oracle."""
+    w = inputs.WORKLOADS["wan1.3b_6x_720p"]
+    s = w.steps[0]
+    ix = build_index(w, s)
+    host, info = ix.copy_host(), ix.info()
+    p = orc.pattern(w.T, w.W, w.a, s)
+    indptr, indices, flags = orc.tile_index(w.T, w.P, w.tile, w.tile, p.A)
+    assert info.N == 435600 and info.nq == 3404 and info.nnz == len(indices)
+    assert np.array_equal(host.indptr, indptr) and np.array_equal(host.indices, indices)
+    assert np.array_equal(host.flags, flags) and np.array_equal(host.a_bits, p.a_bits())
+    ix.destroy()
+    rows = inputs.sample_rows(w, n_uniform=768, n_edge=256)
+    run_case(w, "tcgen05", (s,), rows=rows, layer=w.layers[0])
+
+
+@pytest.mark.slow
 def test_wan6x_probe_and_all_tiles():
     w = inputs.WORKLOADS["wan1.3b_6x"]
     probe_check(w, "tcgen05", (0, 25))
