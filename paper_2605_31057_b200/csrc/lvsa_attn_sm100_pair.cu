@@ -48,7 +48,8 @@ template <int NS>
 struct SmemP {
     static constexpr int Q_OFF = 0;                            // 32 KB
     static constexpr int RING_OFF = TILE_BYTES;                // NS x 16 KB
-    static constexpr int BAR_OFF = RING_OFF + NS * STAGE_BYTES;
+    static constexpr int OUT_OFF = RING_OFF + NS * STAGE_BYTES;  // 32 KB: output staging, two [128 rows][128 B] spans
+    static constexpr int BAR_OFF = OUT_OFF + TILE_BYTES;
     // barriers (8 B each).  "L": only the leader's copy is used (arrivals come from both CTAs).
     static constexpr int Q_FULL = 0 /*L*/, Q_EMPTY = 1, S_FULL = 2 /*3*/, PA_FULL = 5 /*3, L*/, PB_FULL = 8 /*3, L*/,
                          PV_DONE = 11 /*2*/, O_FULL = 13, O_FREE = 14 /*L*/, KV_FULL = 15 /*NS, L*/,
@@ -84,18 +85,19 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1)
 lvsa_attn_sm100_pair_kernel(const __grid_constant__ CUtensorMap tmap_q,
                             const __grid_constant__ CUtensorMap tmap_k,   // box 64 rows
                             const __grid_constant__ CUtensorMap tmap_v,   // box 128 rows
-                            __nv_bfloat16 *__restrict__ out, float *__restrict__ lse,
+                            const __grid_constant__ CUtensorMap tmap_o,   // out, box 128 rows x 64 channels
+                            float *__restrict__ lse,
                             const int32_t *__restrict__ item_ptr, const int32_t *__restrict__ item_tiles,
                             const int32_t *__restrict__ item_col0,
                             const uint32_t *__restrict__ a_bits, int words, long long N, int P, int T,
-                            int H, int h0, int hc, int n_items, long long n_work, long long sn, long long sh,
-                            long long sb, float scale_log2) {
+                            int H, int h0, int hc, int n_items, long long n_work, float scale_log2) {
     using SM = SmemP<NS>;
     extern __shared__ __align__(1024) uint8_t smem_raw[];
     const uint32_t base = smem_u32(smem_raw);
     if ((base & 1023u) != 0u) __trap();   // SWIZZLE_128B tiles and UMMA descriptors need 1024 B
     uint8_t *base_gen = smem_raw;
     const uint32_t sQ = base + SM::Q_OFF, sRing = base + SM::RING_OFF, sBar = base + SM::BAR_OFF;
+    const uint32_t sOut = base + SM::OUT_OFF;
     auto bar = [&](int i) { return sBar + 8u * (uint32_t)i; };
     volatile uint32_t *tmem_slot_gen = reinterpret_cast<volatile uint32_t *>(base_gen + SM::TMEM_SLOT_OFF);
 
@@ -114,7 +116,7 @@ lvsa_attn_sm100_pair_kernel(const __grid_constant__ CUtensorMap tmap_q,
         mbar_init(bar(SM::O_FREE), 16);             // 8 warps x 2 CTAs
         for (int s = 0; s < NS; ++s) { mbar_init(bar(SM::KV_FULL + s), 1); mbar_init(bar(SM::KV_EMPTY + s), 1); }
         fence_barrier_init();
-        prefetch_tmap(&tmap_q); prefetch_tmap(&tmap_k); prefetch_tmap(&tmap_v);
+        prefetch_tmap(&tmap_q); prefetch_tmap(&tmap_k); prefetch_tmap(&tmap_v); prefetch_tmap(&tmap_o);
     }
     if (warp == 9) tmem_alloc_pair<512>(base + SM::TMEM_SLOT_OFF);
     tc_fence_before();
@@ -142,6 +144,7 @@ lvsa_attn_sm100_pair_kernel(const __grid_constant__ CUtensorMap tmap_q,
         auto tok_wait = [&]() { asm volatile("bar.sync %0, 256;" ::"r"(1 + w) : "memory"); };
         auto tok_pass = [&]() { asm volatile("bar.arrive %0, 256;" ::"r"(1 + (w ^ 1)) : "memory"); };
         auto pair_sync = [&]() { asm volatile("bar.sync 3, 256;" ::: "memory"); };
+        auto wg_sync = [&]() { asm volatile("bar.sync %0, 128;" ::"r"(4 + w) : "memory"); };    // my warpgroup only
         const uint32_t pa_full0 = map_to_cta(bar(SM::PA_FULL), 0);           // the leader's barriers
         const uint32_t pb_full0 = map_to_cta(bar(SM::PB_FULL), 0);
         const uint32_t ofree = map_to_cta(bar(SM::O_FREE), 0);
@@ -342,32 +345,43 @@ lvsa_attn_sm100_pair_kernel(const __grid_constant__ CUtensorMap tmap_q,
                 pair_sync();   // m_ref and the exchange slots are free again for the next item
                 const bool row_ok = my_row < N;
                 const float inv = 1.f / l_tot;
-                __nv_bfloat16 *orow = out + (size_t)b * sb + (size_t)(row_ok ? my_row : 0) * sn + (size_t)h * sh + w * CH;
+                // My 64 channels go to my warpgroup's span of the staging buffer, [128 rows][128 B] in the
+                // SWIZZLE_128B layout of the output tensor map (16-byte chunk j of row r sits at chunk
+                // j ^ (r & 7): conflict-free for the 8 rows a store phase covers), and one TMA store per
+                // warpgroup writes the span out (rows >= N are clipped by the tensor map).
+                if (rw == 0) tma_store_wait_read();        // the previous item's store has read the span
+                wg_sync();
+                const uint32_t srow = sOut + (uint32_t)w * SPAN_BYTES + (uint32_t)rw * 128u;
 #pragma unroll
                 for (int c = 0; c < 2; ++c) {
                     uint32_t r[32];
                     tmem_ld_32x32b_x32(tOh + c * 32, r);
                     tmem_wait_ld();
-                    uint4 *dst = reinterpret_cast<uint4 *>(orow + c * 32);
 #pragma unroll
                     for (int x = 0; x < 4; ++x) {
-                        uint4 v;
-                        v.x = pack_bf16x2(__uint_as_float(r[8 * x + 0]) * inv, __uint_as_float(r[8 * x + 1]) * inv);
-                        v.y = pack_bf16x2(__uint_as_float(r[8 * x + 2]) * inv, __uint_as_float(r[8 * x + 3]) * inv);
-                        v.z = pack_bf16x2(__uint_as_float(r[8 * x + 4]) * inv, __uint_as_float(r[8 * x + 5]) * inv);
-                        v.w = pack_bf16x2(__uint_as_float(r[8 * x + 6]) * inv, __uint_as_float(r[8 * x + 7]) * inv);
-                        if (row_ok) dst[x] = v;
+                        const uint32_t v0 = pack_bf16x2(__uint_as_float(r[8 * x + 0]) * inv, __uint_as_float(r[8 * x + 1]) * inv);
+                        const uint32_t v1 = pack_bf16x2(__uint_as_float(r[8 * x + 2]) * inv, __uint_as_float(r[8 * x + 3]) * inv);
+                        const uint32_t v2 = pack_bf16x2(__uint_as_float(r[8 * x + 4]) * inv, __uint_as_float(r[8 * x + 5]) * inv);
+                        const uint32_t v3 = pack_bf16x2(__uint_as_float(r[8 * x + 6]) * inv, __uint_as_float(r[8 * x + 7]) * inv);
+                        st_shared_v4(srow + (uint32_t)(((4 * c + x) ^ (rw & 7)) * 16), v0, v1, v2, v3);
                     }
                 }
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive_cluster(ofree);
+                fence_proxy_async_smem();                  // my generic-proxy writes, before the async-proxy read
+                wg_sync();
+                if (rw == 0) {
+                    tma_store_4d(&tmap_o, sOut + (uint32_t)w * SPAN_BYTES, w * CH, h, (int)((long long)item * 256 + rank * 128), b);
+                    tma_store_commit();
+                }
                 if (w == 0 && row_ok && lse != nullptr)
                     lse[((size_t)b * H + h) * N + my_row] = m_run * 0.6931471805599453f + __logf(l_tot);
             }
         }
         // drain the token that is left on one of the two barriers
         if ((tc & 1u) == (uint32_t)w) tok_wait();
+        if (rw == 0) tma_store_wait_all();                 // my output stores have left shared memory
     } else {
         reg_dec<88>();
         if (warp == 8 && lane == 0) {
@@ -562,22 +576,22 @@ lvsa_status_t lvsa_attn_sm100_pair_launch_heads(const lvsa_index *ix, const void
                                                 void *out, float *lse, int h0, int hc, cudaStream_t stream) {
     constexpr int NS = LVSA_PAIR_STAGES;
     using SM = SmemP<NS>;
-    CUtensorMap mq, mk, mv;
+    CUtensorMap mq, mk, mv, mo;
     lvsa_status_t st;
     if ((st = lvsa_make_tmap_bf16(&mq, q, ix, 128)) != LVSA_OK) return st;
     if ((st = lvsa_make_tmap_bf16(&mk, k, ix, 64)) != LVSA_OK) return st;
     if ((st = lvsa_make_tmap_bf16(&mv, v, ix, BT)) != LVSA_OK) return st;
+    if ((st = lvsa_make_tmap_bf16(&mo, out, ix, 128)) != LVSA_OK) return st;
     if ((st = lvsa_attn_sm100_pair_prepare(ix->device)) != LVSA_OK) return st;
     const long long n_work = (long long)ix->n_items * hc * ix->p.B;
     long long n_pairs = g_pair_n_sm[ix->device] / 2;
-    const lvsa_strides sd = lvsa_layout_strides(ix);
     if (n_work < n_pairs) n_pairs = n_work;
     const float scale_log2 = ix->p.softmax_scale * 1.4426950408889634f;
     auto kern = ix->p.kv_tiling == LVSA_KV_TILES_FRAME_ALIGNED ? lvsa_attn_sm100_pair_kernel<NS, true>
                                                                : lvsa_attn_sm100_pair_kernel<NS, false>;
     kern<<<(unsigned)(2 * n_pairs), NTHREADS, SM::BYTES, stream>>>(
-        mq, mk, mv, (__nv_bfloat16 *)out, lse, ix->d_item_ptr, ix->d_item_tiles, ix->d_item_col0, ix->d_abits, ix->words,
-        (long long)ix->N, ix->p.P, ix->Tf, ix->p.H, h0, hc, (int)ix->n_items, n_work, sd.n, sd.h, sd.b, scale_log2);
+        mq, mk, mv, mo, lse, ix->d_item_ptr, ix->d_item_tiles, ix->d_item_col0, ix->d_abits, ix->words,
+        (long long)ix->N, ix->p.P, ix->Tf, ix->p.H, h0, hc, (int)ix->n_items, n_work, scale_log2);
     LVSA_CUDA_TRY(cudaGetLastError());
     return LVSA_OK;
 }
