@@ -116,11 +116,6 @@ def dist_setup(n_gpus: int):
     return replicas.setup("nccl")
 
 
-def exact_flops(w, A) -> float:
-    """Eq. 2 work: 4 d flops per (query row, head, attended key)."""
-    return float(A.sum()) * w.P * w.P * 4.0 * w.d * w.H * w.B
-
-
 # ------------------------------------------------------------------------------------------
 def run_ours(args):
     from paper_2605_31057_b200 import binding

@@ -198,10 +198,16 @@ __global__ void lvsa_tiles_kernel(long long N, int P, int Tv, int Tf, int Bq, in
     }
     if (!FILL && tid == 0) { counts[i0] = run[0]; if (has1) counts[i1] = run[1]; icounts[g] = run[2]; }
     if (FILL) {
+        // one global atomic per block and counter (all blocks add to the same two addresses)
+        __shared__ int part_s;
+        __shared__ unsigned long long cols_s;
+        if (tid == 0) { part_s = 0; cols_s = 0ull; }
+        __syncthreads();
         n_part = __reduce_add_sync(0xffffffffu, n_part);
-        if (lane == 0 && n_part) atomicAdd(&meta[1], n_part);
         for (int o = 16; o > 0; o >>= 1) n_cols += __shfl_xor_sync(0xffffffffu, n_cols, o);
-        if (lane == 0 && n_cols) atomicAdd(kept_cols, (unsigned long long)n_cols);
+        if (lane == 0) { if (n_part) atomicAdd(&part_s, n_part); if (n_cols) atomicAdd(&cols_s, (unsigned long long)n_cols); }
+        __syncthreads();
+        if (tid == 0) { if (part_s) atomicAdd(&meta[1], part_s); if (cols_s) atomicAdd(kept_cols, cols_s); }
     }
 }
 
