@@ -134,7 +134,10 @@ def run_ours(args):
     stream = torch.cuda.current_stream()
     steps_cycle = list(w.steps) if w.steps else [0]
 
+    kernel_of = {"default": binding.KERNEL_AUTO, "quad": binding.KERNEL_TCGEN05_QUAD, "v0": binding.KERNEL_TCGEN05_V0}
+
     def build(s, **kw):
+        kw.setdefault("kernel", kernel_of[args.kernel])
         return binding.lvsa_build_block_index_ex(
             stream=stream.cuda_stream, T=w.T, P=w.P, H=w.H, d=w.d, B=w.B, window=w.W, anchors=w.a,
             step=s, layer=w.layers[0] if w.layers else 0, n_text=w.n_text, initial_anchors=w.k0, **kw)
@@ -217,7 +220,7 @@ def run_ours(args):
     # ---- the frame-aligned kv tiling (row f4, reading R25) on the same inputs: same timing recipe as
     # the headline kernel (back to back inside a loop, and alone after an idle gap)
     fa_line = None
-    if rank == 0 and not args.no_dense:
+    if rank == 0 and not args.no_dense and args.kernel == "default":
         s_fa = steps_cycle[min(1, len(steps_cycle) - 1)]
         ix_fa = build(s_fa, kv_tiling=binding.KV_TILES_FRAME_ALIGNED)
         i_fa = ix_fa.info()
@@ -241,6 +244,34 @@ def run_ours(args):
                    "tflops_computed": round(tile_flop(i_fa.kept_cols) / (fa_ms * 1e-3) / 1e12, 1),
                    "note": "fewer computed columns, more tile visits: no gain, the kernel's time follows the tile visits (DESIGN.md 7.2c)"}
         ix_fa.destroy()
+
+    # ---- the 4-CTA-cluster variant (row f4: K/V shared by two MMA pairs through one multicast load):
+    # same loops, alternating with the default kernel, SM clock sampled during each loop
+    quad_line = None
+    if rank == 0 and not args.no_dense and w.d == 128 and args.kernel == "default":
+        s_q = steps_cycle[min(1, len(steps_cycle) - 1)]
+        ix_q = build(s_q, kernel=binding.KERNEL_TCGEN05_QUAD)
+
+        def timed(ix, n):
+            smp = ClockSampler(local)
+            smp.start()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            for _ in range(3):
+                binding.lvsa_attn_fwd(q, k, v, ix, out, lse, stream.cuda_stream)
+            a.record(stream)
+            for _ in range(n):
+                binding.lvsa_attn_fwd(q, k, v, ix, out, lse, stream.cuda_stream)
+            b.record(stream)
+            torch.cuda.synchronize()
+            return a.elapsed_time(b) / n, smp.stop()["sm_mhz"]
+        n_q = max(10, min(args.steps, 20))
+        r4 = [timed(ix, n_q) for ix in (ix_q, ix_k, ix_q, ix_k)]
+        mhz = lambda a, b: None if a is None or b is None else round(0.5 * (a + b), 0)
+        quad_line = {"ms": round(0.5 * (r4[0][0] + r4[2][0]), 4), "ms_pair_kernel_same_loops": round(0.5 * (r4[1][0] + r4[3][0]), 4),
+                     "sm_mhz": mhz(r4[0][1], r4[2][1]), "sm_mhz_pair_kernel": mhz(r4[1][1], r4[3][1]),
+                     "grid_ctas": ix_q.grid(), "grid_ctas_pair_kernel": ix_k.grid(),
+                     "note": "K/V loaded once per 4-CTA cluster (half the L2 -> SM traffic); 4-CTA clusters cannot cover every SM (DESIGN.md 7.2d)"}
+        ix_q.destroy()
 
     # ---- index build alone (a1-a5): 4 kernels, enqueue only; device time by events, host time by clock
     torch.cuda.synchronize()
@@ -387,7 +418,7 @@ def run_ours(args):
             "data": "synthetic (i.i.d. N(0,1) bf16, seeded Philox; stands in for Wan 2.1 latents)",
             "config": {"workload": args.workload, "T": w.T, "P": w.P, "N": w.N, "H": w.H, "d": w.d,
                        "B": w.B, "tile": w.tile, "window": w.W, "anchors": w.a,
-                       "steps_cycled": steps_cycle, "nnz_mean": nnz_mean,
+                       "steps_cycled": steps_cycle, "nnz_mean": nnz_mean, "kernel": args.kernel,
                        "l2": "inputs (3 x %.0f MB) exceed the 126 MB L2; no flush" % (q.numel() * 2 / 1e6),
                        "parallelism": "replicas only (one independent call per GPU)" if world > 1 else "1 GPU"},
             "ms_per_attention_call": round(kern_ms, 4),
@@ -403,6 +434,7 @@ def run_ours(args):
                 "speedup_lvsa_vs_all_tiles": round(dense_ms / kern_ms, 3),
                 "tflops": round(tile_flop(dense_cols) / (dense_ms * 1e-3) / 1e12, 1)},
             "frame_aligned_kv_tiles": fa_line,
+            "quad_cluster_multicast": quad_line,
             "schedule": sched_line,
             "roofline": {"bound": "tensor", "achieved": round(achieved, 2), "peak": peak_sus,
                          "unit": "TFLOP/s", "frac": round(achieved / peak_sus, 4), "traffic": traffic,
@@ -492,6 +524,8 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-dense", action="store_true")
     ap.add_argument("--no-schedule", action="store_true")
+    ap.add_argument("--kernel", default="default", choices=["default", "quad", "v0"],
+                    help="attention kernel of the timed steps (default: the CTA-pair kernel); for A/B runs and ncu captures")
     ap.add_argument("--window", type=int, default=None, help="override W of the workload (sensitivity runs)")
     ap.add_argument("--anchors", type=int, default=None, help="override a = C - (2W+1) of the workload")
     args = ap.parse_args()

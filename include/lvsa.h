@@ -41,8 +41,12 @@ enum { LVSA_DTYPE_BF16 = 0, LVSA_DTYPE_FP32 = 1 };             /* element type o
 /* LVSA_KERNEL_TCGEN05: the production tensor-core kernel (d = 128: persistent CTA-pair kernel,
  * cta_group::2; d = 64: the one-CTA-per-item kernel).  LVSA_KERNEL_TCGEN05_V0: the simple
  * one-CTA-per-item tcgen05 kernel for d = 128 too (a second implementation of the same maths, kept
- * as an A/B and cross-check variant; same results within the stated tolerance). */
-enum { LVSA_KERNEL_AUTO = 0, LVSA_KERNEL_SIMT = 1, LVSA_KERNEL_TCGEN05 = 2, LVSA_KERNEL_TCGEN05_V0 = 3 };
+ * as an A/B and cross-check variant; same results within the stated tolerance).
+ * LVSA_KERNEL_TCGEN05_QUAD (d = 128, token-0 kv tiles): the CTA-pair kernel run as clusters of FOUR CTAs,
+ * two MMA pairs working on adjacent work items that receive every K/V tile from ONE TMA load
+ * (multicast), which halves the L2 -> SM traffic. */
+enum { LVSA_KERNEL_AUTO = 0, LVSA_KERNEL_SIMT = 1, LVSA_KERNEL_TCGEN05 = 2, LVSA_KERNEL_TCGEN05_V0 = 3,
+       LVSA_KERNEL_TCGEN05_QUAD = 4 };
 /* Memory order of q, k, v, out (PAPER.md:31 fixes only N = T*P, not the order of the axes):
  * NHD = [B, N, H, d] (default), HND = [B, H, N, d]; d is always fastest.  lse is [B, H, N] in both. */
 enum { LVSA_LAYOUT_NHD = 0, LVSA_LAYOUT_HND = 1 };
@@ -226,6 +230,12 @@ lvsa_status_t lvsa_index_copy_kv_tiles(const lvsa_index_t *index, int32_t *col0,
 
 /* Number of kernels lvsa_attn_fwd enqueues per call for this index (bench.py's gpu_launches). */
 int lvsa_attn_fwd_launches(const lvsa_index_t *index);
+
+/* Number of CTAs the (persistent) tensor-core attention kernel is launched with for this index on its
+ * device: 2 x the CTA pairs, or 4 x the 4-CTA clusters that can be resident at once
+ * (LVSA_KERNEL_TCGEN05_QUAD; a cluster needs four SMs of one GPC, so some SMs stay idle).  0 for the
+ * kernels that launch one CTA per work item, -1 on error. */
+int lvsa_attn_fwd_grid(const lvsa_index_t *index);
 
 /* Last error message of the calling thread ("" if none).  Never NULL. */
 const char *lvsa_last_error(void);

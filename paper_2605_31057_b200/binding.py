@@ -20,7 +20,7 @@ ALL_TILES = -1
 TILE_FULL, TILE_PARTIAL = 0, 1
 TIE_LO, TIE_HI = 0, 1
 DTYPE_BF16, DTYPE_FP32 = 0, 1
-KERNEL_AUTO, KERNEL_SIMT, KERNEL_TCGEN05, KERNEL_TCGEN05_V0 = 0, 1, 2, 3
+KERNEL_AUTO, KERNEL_SIMT, KERNEL_TCGEN05, KERNEL_TCGEN05_V0, KERNEL_TCGEN05_QUAD = 0, 1, 2, 3, 4
 LAYOUT_NHD, LAYOUT_HND = 0, 1
 KV_TILES_TOKEN0, KV_TILES_FRAME_ALIGNED = 0, 1
 KV_PAD = 32
@@ -54,7 +54,7 @@ class IndexInfo(C.Structure):
 
 EXPORTS = ("lvsa_build_block_index", "lvsa_build_block_index_ex", "lvsa_attn_fwd",
            "lvsa_attn_fwd_host", "lvsa_index_destroy", "lvsa_index_info", "lvsa_index_copy_host",
-           "lvsa_index_copy_kv_tiles", "lvsa_attn_fwd_launches", "lvsa_workspace_release", "lvsa_schedule_create",
+           "lvsa_index_copy_kv_tiles", "lvsa_attn_fwd_launches", "lvsa_attn_fwd_grid", "lvsa_workspace_release", "lvsa_schedule_create",
            "lvsa_schedule_num_phases", "lvsa_schedule_index", "lvsa_schedule_attn_fwd", "lvsa_schedule_destroy", "lvsa_last_error", "lvsa_version")
 
 _lib = None
@@ -82,6 +82,8 @@ def lib() -> C.CDLL:
         L.lvsa_index_copy_host.argtypes = [C.c_void_p] * 7
         L.lvsa_index_copy_kv_tiles.restype = C.c_int
         L.lvsa_index_copy_kv_tiles.argtypes = [C.c_void_p] * 3
+        L.lvsa_attn_fwd_grid.restype = C.c_int
+        L.lvsa_attn_fwd_grid.argtypes = [C.c_void_p]
         L.lvsa_attn_fwd_launches.restype = C.c_int
         L.lvsa_attn_fwd_launches.argtypes = [C.c_void_p]
         L.lvsa_workspace_release.restype = None
@@ -163,6 +165,10 @@ class BlockIndex:
         _check(lib().lvsa_index_copy_kv_tiles(self.handle, col0.ctypes.data_as(C.c_void_p),
                                               width.ctypes.data_as(C.c_void_p)))
         return col0, width
+
+    def grid(self) -> int:
+        """CTAs of the persistent attention launch for this index (0: one CTA per work item)."""
+        return int(lib().lvsa_attn_fwd_grid(self.handle))
 
     def launches(self) -> int:
         return int(lib().lvsa_attn_fwd_launches(self.handle))

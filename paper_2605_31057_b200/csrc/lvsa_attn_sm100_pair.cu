@@ -71,7 +71,6 @@ template <int REGS> __device__ __forceinline__ void reg_dec() { asm volatile("se
 
 template <int V> struct StaticInt { __device__ constexpr operator int() const { return V; } };
 
-__device__ __forceinline__ int entry_state(int entry, int w) { return (entry >> (LVSA_ITEM_J_BITS + 2 * w)) & 3; }
 // 32-column chunks of the kv tile that are computed: 4 for a 128-column tile, fewer for a narrow
 // frame-aligned tile (reading R25)
 __device__ __forceinline__ int entry_chunks(int entry) { return (int)((uint32_t)entry >> LVSA_ITEM_W_SHIFT) + 1; }
@@ -80,8 +79,18 @@ __device__ __forceinline__ int entry_chunks(int entry) { return (int)((uint32_t)
 // alone describes it and the widths are compile-time constants.  VARW = true: frame-aligned kv tiles
 // (LVSA_KV_TILES_FRAME_ALIGNED, reading R25): the first token comes from item_col0[] and the width
 // (32 .. 128 columns) from the entry, in the producer, the issuer and the softmax warps.
-template <int NS, bool VARW>
-__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1)
+//
+// MODE_QUAD: clusters of FOUR CTAs = two MMA pairs working on the two work items of a quad of adjacent
+// q tiles (token-0 tiles).  Every K/V tile is loaded ONCE per cluster: CTA r of pair 0 issues the TMA
+// load of "its" half with a multicast mask naming CTA r of both pairs, so the same bytes land at the
+// same shared-memory offset of both, and each destination's completion is counted on the FULL barrier
+// of its own pair's leader (cta_group::2 load, barrier address with the peer bit cleared).  The two
+// pairs walk the quad's union list in lock step as far as the ring goes: a stage is refilled when the
+// MMAs of BOTH pairs have read it (KV_EMPTY takes one commit from each issuer, multicast to all four
+// CTAs).  Everything else (Q, S/P/O, softmax, epilogue) stays private to a pair.
+enum { MODE_TOKEN0 = 0, MODE_VARW = 1, MODE_QUAD = 2 };
+template <int NS, int MODE>
+__global__ void __cluster_dims__(MODE == MODE_QUAD ? 4 : 2, 1, 1) __launch_bounds__(NTHREADS, 1)
 lvsa_attn_sm100_pair_kernel(const __grid_constant__ CUtensorMap tmap_q,
                             const __grid_constant__ CUtensorMap tmap_k,   // box 64 rows
                             const __grid_constant__ CUtensorMap tmap_v,   // box 128 rows
@@ -92,6 +101,8 @@ lvsa_attn_sm100_pair_kernel(const __grid_constant__ CUtensorMap tmap_q,
                             const uint32_t *__restrict__ a_bits, int words, long long N, int P, int T,
                             int H, int h0, int hc, int n_items, long long n_work, float scale_log2) {
     using SM = SmemP<NS>;
+    constexpr bool VARW = MODE == MODE_VARW, QUAD = MODE == MODE_QUAD;
+    constexpr int CL = QUAD ? 4 : 2;                   // CTAs per cluster
     extern __shared__ __align__(1024) uint8_t smem_raw[];
     const uint32_t base = smem_u32(smem_raw);
     if ((base & 1023u) != 0u) __trap();   // SWIZZLE_128B tiles and UMMA descriptors need 1024 B
@@ -102,8 +113,17 @@ lvsa_attn_sm100_pair_kernel(const __grid_constant__ CUtensorMap tmap_q,
     volatile uint32_t *tmem_slot_gen = reinterpret_cast<volatile uint32_t *>(base_gen + SM::TMEM_SLOT_OFF);
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, wg = tid >> 7;
-    const uint32_t rank = cluster_ctarank();           // 0 = leader; also the q tile of the item I own
-    const long long pair = blockIdx.x >> 1, n_pairs = gridDim.x >> 1;
+    const uint32_t crank = cluster_ctarank();
+    const uint32_t rank = crank & 1u;                  // 0 = leader of my pair; also the q tile of the item I own
+    const uint32_t pid = QUAD ? (crank >> 1) : 0u;     // my pair inside the cluster
+    const uint32_t lead = crank & ~1u;                 // cluster rank of my pair's leader
+    const uint16_t pair_mask = (uint16_t)(3u << (2u * pid));              // commit targets: my pair
+    const uint16_t ring_mask = QUAD ? (uint16_t)0xF : pair_mask;          // ... or every CTA that shares the ring
+    const long long pair = blockIdx.x / CL, n_pairs = gridDim.x / CL;     // cluster index / number of clusters
+    // which list entry bits hold MY q tile's state, and the rows my pair owns in work unit `item`
+    constexpr int J_MASK = QUAD ? LVSA_QUAD_J_MASK : LVSA_ITEM_J_MASK;
+    const int st_shift = QUAD ? LVSA_QUAD_J_BITS + 2 * (int)(2u * pid + rank) : LVSA_ITEM_J_BITS + 2 * (int)rank;
+    auto unit_row0 = [&](int item) { return ((long long)(QUAD ? 2 * item + (int)pid : item)) * 256 + (long long)rank * 128; };
 
     if (warp == 8 && lane == 0) {
         mbar_init(bar(SM::Q_FULL), 1); mbar_init(bar(SM::Q_EMPTY), 1);
@@ -114,7 +134,7 @@ lvsa_attn_sm100_pair_kernel(const __grid_constant__ CUtensorMap tmap_q,
         }
         mbar_init(bar(SM::PV_DONE), 1); mbar_init(bar(SM::PV_DONE + 1), 1); mbar_init(bar(SM::O_FULL), 1);
         mbar_init(bar(SM::O_FREE), 16);             // 8 warps x 2 CTAs
-        for (int s = 0; s < NS; ++s) { mbar_init(bar(SM::KV_FULL + s), 1); mbar_init(bar(SM::KV_EMPTY + s), 1); }
+        for (int s = 0; s < NS; ++s) { mbar_init(bar(SM::KV_FULL + s), 1); mbar_init(bar(SM::KV_EMPTY + s), QUAD ? 2 : 1); }
         fence_barrier_init();
         prefetch_tmap(&tmap_q); prefetch_tmap(&tmap_k); prefetch_tmap(&tmap_v); prefetch_tmap(&tmap_o);
     }
@@ -145,16 +165,16 @@ lvsa_attn_sm100_pair_kernel(const __grid_constant__ CUtensorMap tmap_q,
         auto tok_pass = [&]() { asm volatile("bar.arrive %0, 256;" ::"r"(1 + (w ^ 1)) : "memory"); };
         auto pair_sync = [&]() { asm volatile("bar.sync 3, 256;" ::: "memory"); };
         auto wg_sync = [&]() { asm volatile("bar.sync %0, 128;" ::"r"(4 + w) : "memory"); };    // my warpgroup only
-        const uint32_t pa_full0 = map_to_cta(bar(SM::PA_FULL), 0);           // the leader's barriers
-        const uint32_t pb_full0 = map_to_cta(bar(SM::PB_FULL), 0);
-        const uint32_t ofree = map_to_cta(bar(SM::O_FREE), 0);
+        const uint32_t pa_full0 = map_to_cta(bar(SM::PA_FULL), lead);        // my pair leader's barriers
+        const uint32_t pb_full0 = map_to_cta(bar(SM::PB_FULL), lead);
+        const uint32_t ofree = map_to_cta(bar(SM::O_FREE), lead);
         if (w == 1) tok_pass();     // the first token: tile 0 belongs to warpgroup 0
         uint32_t tc = 0;            // kv tiles of this CTA so far (all items); tile tc belongs to warpgroup tc & 1
         uint32_t oc = 0;            // items finished
         for (long long work = pair; work < n_work; work += n_pairs) {
             const int item = (int)(work % n_items);
             const int bh = (int)(work / n_items), h = h0 + bh % hc, b = bh / hc;   // heads [h0, h0 + hc) of H
-            const long long my_row = (long long)item * 256 + rank * 128 + rw;
+            const long long my_row = unit_row0(item) + rw;
             const int fq = (int)min((long long)(T - 1), my_row / P);
             const uint32_t *arow = a_bits + (size_t)fq * words;
             const int e0 = item_ptr[item], e1 = item_ptr[item + 1];
@@ -167,9 +187,9 @@ lvsa_attn_sm100_pair_kernel(const __grid_constant__ CUtensorMap tmap_q,
                 const uint32_t t_me = tc + (uint32_t)(e - e0);               // running index of this tile
                 const int entry = entry_nx;
                 // first token of the kv tile (PARTIAL tiles need it) and its 32-column chunks
-                const int tile_col0 = VARW ? col0_nx : (entry & LVSA_ITEM_J_MASK) * BT;
+                const int tile_col0 = VARW ? col0_nx : (entry & J_MASK) * BT;
                 if (e + 2 < e1) { entry_nx = __ldg(item_tiles + e + 2); if (VARW) col0_nx = __ldg(item_col0 + e + 2); }
-                const int st = entry_state(entry, (int)rank);
+                const int st = (entry >> st_shift) & 3;
                 const int nch = VARW ? entry_chunks(entry) : 4;
                 const bool first = (e == e0);
 
@@ -372,7 +392,7 @@ lvsa_attn_sm100_pair_kernel(const __grid_constant__ CUtensorMap tmap_q,
                 fence_proxy_async_smem();                  // my generic-proxy writes, before the async-proxy read
                 wg_sync();
                 if (rw == 0) {
-                    tma_store_4d(&tmap_o, sOut + (uint32_t)w * SPAN_BYTES, w * CH, h, (int)((long long)item * 256 + rank * 128), b);
+                    tma_store_4d(&tmap_o, sOut + (uint32_t)w * SPAN_BYTES, w * CH, h, (int)unit_row0(item), b);
                     tma_store_commit();
                 }
                 if (w == 0 && row_ok && lse != nullptr)
@@ -389,31 +409,46 @@ lvsa_attn_sm100_pair_kernel(const __grid_constant__ CUtensorMap tmap_q,
             // Loads MY half of every operand; completion bytes are counted on the LEADER's barriers.
             // The leader arms each barrier with the bytes of both halves.  Ring order = the order the
             // issuer consumes: K(0), K(1), then per tile j: K(j+2), V(j).
-            const uint32_t q_full_L = map_to_cta(bar(SM::Q_FULL), 0);
+            const uint32_t q_full_L = map_to_cta(bar(SM::Q_FULL), lead);
             uint32_t kv_it = 0, qi = 0;
             // col0 = first token of the kv tile; nt = its computed columns.  K: CTA r supplies columns
             // [r nt/2, (r+1) nt/2) of S, i.e. kv rows col0 + r nt/2 ... (the 64-row box over-reads for a
             // narrow tile; the MMA uses the first nt/2 rows).  V: all rows of the tile, my 64 channels.
             auto push = [&](const CUtensorMap *tm, bool is_k, int e, int h, int b) {
-                const int col0 = VARW ? __ldg(item_col0 + e) : (__ldg(item_tiles + e) & LVSA_ITEM_J_MASK) * BT;
+                const int col0 = VARW ? __ldg(item_col0 + e) : (__ldg(item_tiles + e) & J_MASK) * BT;
                 const int nt = VARW ? 32 * entry_chunks(__ldg(item_tiles + e)) : BT;
                 const uint32_t stage = kv_it % NS, n = kv_it / NS;
                 mbar_wait(bar(SM::KV_EMPTY + stage), (n & 1u) ^ 1u);
                 if (rank == 0) mbar_expect_tx(bar(SM::KV_FULL + stage), 2 * STAGE_BYTES);
                 const uint32_t dst = sRing + stage * STAGE_BYTES;
-                const uint32_t full_L = map_to_cta(bar(SM::KV_FULL + stage), 0);
-                if (is_k) {   // kv rows [col0 + 64 rank, +64), channels [0,64) and [64,128): two 8 KB spans
-                    tma_load_4d_pair(dst, tm, full_L, 0, h, col0 + (nt / 2) * (int)rank, b);
-                    tma_load_4d_pair(dst + 8192, tm, full_L, 64, h, col0 + (nt / 2) * (int)rank, b);
-                } else {      // channels [64 rank, +64) of all 128 kv rows: one 16 KB span
-                    tma_load_4d_pair(dst, tm, full_L, 64 * (int)rank, h, col0, b);
+                if (QUAD) {
+                    // pair 0 loads for the whole cluster: my half goes to CTA `rank` of both pairs; the barrier
+                    // operand is my own KV_FULL with the peer bit cleared = "the leader of the destination's pair"
+                    if (pid == 0) {
+                        const uint32_t full_rel = bar(SM::KV_FULL + stage) & 0xFEFFFFFFu;
+                        const uint16_t mc = (uint16_t)(0x5u << rank);
+                        if (is_k) {
+                            tma_load_4d_pair_mc(dst, tm, full_rel, mc, 0, h, col0 + 64 * (int)rank, b);
+                            tma_load_4d_pair_mc(dst + 8192, tm, full_rel, mc, 64, h, col0 + 64 * (int)rank, b);
+                        } else {
+                            tma_load_4d_pair_mc(dst, tm, full_rel, mc, 64 * (int)rank, h, col0, b);
+                        }
+                    }
+                } else {
+                    const uint32_t full_L = map_to_cta(bar(SM::KV_FULL + stage), lead);
+                    if (is_k) {   // kv rows [col0 + 64 rank, +64), channels [0,64) and [64,128): two 8 KB spans
+                        tma_load_4d_pair(dst, tm, full_L, 0, h, col0 + (nt / 2) * (int)rank, b);
+                        tma_load_4d_pair(dst + 8192, tm, full_L, 64, h, col0 + (nt / 2) * (int)rank, b);
+                    } else {      // channels [64 rank, +64) of all 128 kv rows: one 16 KB span
+                        tma_load_4d_pair(dst, tm, full_L, 64 * (int)rank, h, col0, b);
+                    }
                 }
                 ++kv_it;
             };
             for (long long work = pair; work < n_work; work += n_pairs) {
                 const int item = (int)(work % n_items);
                 const int bh = (int)(work / n_items), h = h0 + bh % hc, b = bh / hc;   // heads [h0, h0 + hc) of H
-                const long long row0 = (long long)item * 256 + (long long)rank * 128;
+                const long long row0 = unit_row0(item);
                 const int e0 = item_ptr[item], e1 = item_ptr[item + 1];
                 mbar_wait(bar(SM::Q_EMPTY), (qi & 1u) ^ 1u);
                 if (rank == 0) mbar_expect_tx(bar(SM::Q_FULL), 2 * TILE_BYTES);
@@ -448,9 +483,9 @@ lvsa_attn_sm100_pair_kernel(const __grid_constant__ CUtensorMap tmap_q,
                     umma_ss_pair(tmem_base + buf * 128, dQ + (uint64_t)offA,
                                  dRing + (uint64_t)(((stage * STAGE_BYTES) >> 4) + offB), IDESC_S, kk > 0);
                 }
-                umma_commit_pair(bar(SM::S_FULL + buf));
-                umma_commit_pair(bar(SM::KV_EMPTY + stage));
-                if (last_of_item) umma_commit_pair(bar(SM::Q_EMPTY));   // Q is last read by S of the final tile
+                umma_commit_pair(bar(SM::S_FULL + buf), pair_mask);
+                umma_commit_pair(bar(SM::KV_EMPTY + stage), ring_mask);
+                if (last_of_item) umma_commit_pair(bar(SM::Q_EMPTY), pair_mask);   // Q is last read by S of the final tile
             };
             // O += P(buf) V: A = P from TMEM (2 bf16 per column), B = V half (MN-major, 64 channels per
             // CTA = one 128 B span; 16 kv rows = 2048 B per k-block)
@@ -526,18 +561,18 @@ lvsa_attn_sm100_pair_kernel(const __grid_constant__ CUtensorMap tmap_q,
                     tc_fence_after();
                     if (elect_one_sync()) {
                         issue_PV(buf, stageV, j > 0, 1, nt_pv);
-                        umma_commit_pair(bar(SM::PV_DONE + (tc & 1u)));
-                        umma_commit_pair(bar(SM::KV_EMPTY + stageV));
+                        umma_commit_pair(bar(SM::PV_DONE + (tc & 1u)), pair_mask);
+                        umma_commit_pair(bar(SM::KV_EMPTY + stageV), ring_mask);
                     }
                     __syncwarp();
                     nt0 = nt1; nt1 = nt2; nt2 = VARW ? uniform_nt(raw3) : BT;
                 }
                 if (n > 0) {
-                    if (elect_one_sync()) umma_commit_pair(bar(SM::O_FULL));
+                    if (elect_one_sync()) umma_commit_pair(bar(SM::O_FULL), pair_mask);
                     __syncwarp();
                     ++oc;
                 } else if (elect_one_sync()) {
-                    umma_commit_pair(bar(SM::Q_EMPTY));
+                    umma_commit_pair(bar(SM::Q_EMPTY), pair_mask);
                 }
                 __syncwarp();
             }
@@ -556,18 +591,44 @@ lvsa_status_t lvsa_make_tmap_bf16(CUtensorMap *m, const void *base, const lvsa_i
 // One-time setup per DEVICE (the shared-memory attribute and the SM count belong to a device, not
 // to the process); `device` must be the current device.
 static int g_pair_n_sm[LVSA_MAX_DEVICES] = {};
+static int g_quad_clusters[LVSA_MAX_DEVICES] = {};   // 4-CTA clusters that can be resident at once
 lvsa_status_t lvsa_attn_sm100_pair_prepare(int device) {
     if (device < 0 || device >= LVSA_MAX_DEVICES) { lvsa_set_error("device ordinal out of range"); return LVSA_EUNSUPPORTED; }
     if (g_pair_n_sm[device] != 0) return LVSA_OK;
     using SM = SmemP<LVSA_PAIR_STAGES>;
-    LVSA_CUDA_TRY(cudaFuncSetAttribute(lvsa_attn_sm100_pair_kernel<LVSA_PAIR_STAGES, false>,
+    LVSA_CUDA_TRY(cudaFuncSetAttribute(lvsa_attn_sm100_pair_kernel<LVSA_PAIR_STAGES, MODE_TOKEN0>,
                                        cudaFuncAttributeMaxDynamicSharedMemorySize, SM::BYTES));
-    LVSA_CUDA_TRY(cudaFuncSetAttribute(lvsa_attn_sm100_pair_kernel<LVSA_PAIR_STAGES, true>,
+    LVSA_CUDA_TRY(cudaFuncSetAttribute(lvsa_attn_sm100_pair_kernel<LVSA_PAIR_STAGES, MODE_VARW>,
+                                       cudaFuncAttributeMaxDynamicSharedMemorySize, SM::BYTES));
+    LVSA_CUDA_TRY(cudaFuncSetAttribute(lvsa_attn_sm100_pair_kernel<LVSA_PAIR_STAGES, MODE_QUAD>,
                                        cudaFuncAttributeMaxDynamicSharedMemorySize, SM::BYTES));
     int n = 0;
     LVSA_CUDA_TRY(cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, device));
+    // A 4-CTA cluster needs four free SMs of one GPC, so fewer than n / 4 of them may fit at once; the
+    // persistent grid must not be larger than that (a cluster that is not resident would only start
+    // when another one has finished ALL its work).
+    {
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3((unsigned)(n / 4 * 4)); cfg.blockDim = dim3(NTHREADS); cfg.dynamicSmemBytes = SM::BYTES;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = 4; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+        cfg.attrs = at; cfg.numAttrs = 1;
+        int nc = 0;
+        LVSA_CUDA_TRY(cudaOccupancyMaxActiveClusters(&nc, lvsa_attn_sm100_pair_kernel<LVSA_PAIR_STAGES, MODE_QUAD>, &cfg));
+        g_quad_clusters[device] = nc > 0 ? nc : 1;
+    }
     g_pair_n_sm[device] = n;
     return LVSA_OK;
+}
+
+int lvsa_attn_sm100_pair_grid(const lvsa_index *ix, int hc) {
+    const bool quad = ix->p.kernel == LVSA_KERNEL_TCGEN05_QUAD;
+    const int cl = quad ? 4 : 2;
+    const long long n_work = (quad ? ix->n_quads : ix->n_items) * hc * ix->p.B;
+    long long n_clusters = quad ? g_quad_clusters[ix->device] : g_pair_n_sm[ix->device] / cl;
+    if (n_work < n_clusters) n_clusters = n_work;
+    return (int)(cl * n_clusters);
 }
 
 // Heads [h0, h0 + hc) only (all batches): the host entry point pipelines head groups against the
@@ -583,15 +644,19 @@ lvsa_status_t lvsa_attn_sm100_pair_launch_heads(const lvsa_index *ix, const void
     if ((st = lvsa_make_tmap_bf16(&mv, v, ix, BT)) != LVSA_OK) return st;
     if ((st = lvsa_make_tmap_bf16(&mo, out, ix, 128)) != LVSA_OK) return st;
     if ((st = lvsa_attn_sm100_pair_prepare(ix->device)) != LVSA_OK) return st;
-    const long long n_work = (long long)ix->n_items * hc * ix->p.B;
-    long long n_pairs = g_pair_n_sm[ix->device] / 2;
-    if (n_work < n_pairs) n_pairs = n_work;
+    const bool quad = ix->p.kernel == LVSA_KERNEL_TCGEN05_QUAD;
+    const int cl = quad ? 4 : 2;                                             // CTAs per cluster
+    const long long n_units = quad ? ix->n_quads : ix->n_items;             // work units per (head, batch)
+    const long long n_work = n_units * hc * ix->p.B;
+    const long long n_clusters = lvsa_attn_sm100_pair_grid(ix, hc) / cl;
     const float scale_log2 = ix->p.softmax_scale * 1.4426950408889634f;
-    auto kern = ix->p.kv_tiling == LVSA_KV_TILES_FRAME_ALIGNED ? lvsa_attn_sm100_pair_kernel<NS, true>
-                                                               : lvsa_attn_sm100_pair_kernel<NS, false>;
-    kern<<<(unsigned)(2 * n_pairs), NTHREADS, SM::BYTES, stream>>>(
-        mq, mk, mv, mo, lse, ix->d_item_ptr, ix->d_item_tiles, ix->d_item_col0, ix->d_abits, ix->words,
-        (long long)ix->N, ix->p.P, ix->Tf, ix->p.H, h0, hc, (int)ix->n_items, n_work, scale_log2);
+    auto kern = quad ? lvsa_attn_sm100_pair_kernel<NS, MODE_QUAD>
+              : ix->p.kv_tiling == LVSA_KV_TILES_FRAME_ALIGNED ? lvsa_attn_sm100_pair_kernel<NS, MODE_VARW>
+                                                               : lvsa_attn_sm100_pair_kernel<NS, MODE_TOKEN0>;
+    kern<<<(unsigned)(cl * n_clusters), NTHREADS, SM::BYTES, stream>>>(
+        mq, mk, mv, mo, lse, quad ? ix->d_quad_ptr : ix->d_item_ptr, quad ? ix->d_quad_tiles : ix->d_item_tiles,
+        ix->d_item_col0, ix->d_abits, ix->words,
+        (long long)ix->N, ix->p.P, ix->Tf, ix->p.H, h0, hc, (int)n_units, n_work, scale_log2);
     LVSA_CUDA_TRY(cudaGetLastError());
     return LVSA_OK;
 }

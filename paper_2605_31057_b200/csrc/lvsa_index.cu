@@ -211,6 +211,64 @@ __global__ void lvsa_tiles_kernel(long long N, int P, int Tv, int Tf, int Bq, in
     }
 }
 
+// Work lists of the 4-CTA-cluster kernel (LVSA_KERNEL_TCGEN05_QUAD): one block per QUAD of adjacent
+// q tiles (two work items); the list is the union of the kv lists of the four q tiles, each entry
+// tagged with four 2-bit states (token-0 tiling only).  Same ordered compaction as above.
+//   FILL = false: qcounts[u];  FILL = true: quad_tiles at quad_ptr[u].
+template <bool FILL>
+__global__ void lvsa_quads_kernel(long long N, int P, int Tf, int Bq, int Bk, int nq, int nk, int words,
+                                  const uint32_t *__restrict__ a_bits, const int32_t *__restrict__ quad_ptr,
+                                  int32_t *__restrict__ qcounts, int32_t *__restrict__ quad_tiles,
+                                  const int32_t *__restrict__ meta) {
+    __shared__ int warp_tot[32];
+    const int u = blockIdx.x, tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const int nwarps = blockDim.x >> 5;
+    if (FILL && meta[7]) return;
+    int fa[4], fb[4];
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+        const int i = 4 * u + w;
+        const long long r0 = (long long)i * Bq;
+        const long long r1 = min(r0 + Bq, N) - 1;
+        fa[w] = min((int)(min(r0, N - 1) / P), Tf - 1);
+        fb[w] = i < nq ? min((int)(r1 / P), Tf - 1) : fa[w] - 1;   // empty range: no such q tile
+    }
+    int run = 0;
+    const int base = FILL ? quad_ptr[u] : 0;
+    for (int j0 = 0; j0 < nk; j0 += blockDim.x) {
+        const int j = j0 + tid;
+        unsigned st = 0u;   // four 2-bit states
+        if (j < nk) {
+            const long long c0 = (long long)j * Bk;
+            const long long c1 = min(c0 + Bk, N) - 1;
+            const int g0 = min((int)(c0 / P), Tf - 1), g1 = min((int)(c1 / P), Tf - 1);
+            const bool tail = (c0 + Bk > N);
+#pragma unroll
+            for (int w = 0; w < 4; ++w) {
+                bool kept = false, part = tail;
+                for (int tq = fa[w]; tq <= fb[w]; ++tq) {
+                    const uint32_t *row = a_bits + (size_t)tq * words;
+                    for (int tk = g0; tk <= g1; ++tk) {
+                        const bool b = bit_test(row, tk);
+                        kept |= b; part |= !b;
+                    }
+                }
+                st |= (unsigned)(kept ? (part ? LVSA_ST_PARTIAL : LVSA_ST_FULL) : LVSA_ST_SKIP) << (2 * w);
+            }
+        }
+        const unsigned bal = __ballot_sync(0xffffffffu, st != 0u);
+        if (lane == 0) warp_tot[wid] = __popc(bal);
+        __syncthreads();
+        int woff = 0, tot = 0;
+        for (int w = 0; w < nwarps; ++w) { const int c = warp_tot[w]; if (w < wid) woff += c; tot += c; }
+        if (FILL && st != 0u)
+            quad_tiles[base + run + woff + __popc(bal & ((1u << lane) - 1u))] = (int32_t)((unsigned)j | (st << LVSA_QUAD_J_BITS));
+        run += tot;
+        __syncthreads();
+    }
+    if (!FILL && tid == 0) qcounts[u] = run;
+}
+
 // Single-block exclusive scan: out[0..n] from counts[0..n-1]; total also to *total_out.
 // If the total exceeds `cap` (the host's allocation bound) meta[7] is raised and the fill passes
 // write nothing; the host reports it at the next lvsa_index_info / copy_host.
@@ -304,6 +362,16 @@ lvsa_status_t lvsa_index_build_device(lvsa_index *ix, cudaStream_t stream) {
     const size_t o_item_tiles = take(sizeof(int32_t) * (size_t)(ix->cap_item_tiles + 1));
     const size_t o_item_col0 = take(sizeof(int32_t) * (size_t)(ix->cap_item_tiles + 1));
     const size_t o_kept_cols = take(sizeof(unsigned long long));
+    // work lists of the 4-CTA-cluster kernel, built only when that kernel was asked for
+    const bool quads = p.kernel == LVSA_KERNEL_TCGEN05_QUAD;
+    ix->n_quads = quads ? (ix->nq + 3) / 4 : 0;
+    long long per_quad = per_q * 4; if (per_quad > ix->nk) per_quad = ix->nk;
+    ix->cap_quad_tiles = quads ? per_quad * ix->n_quads + text_q * ix->nk : 0;
+    if (ix->cap_quad_tiles >= (1ll << 31)) { lvsa_set_error("index too large for int32 offsets"); return LVSA_EUNSUPPORTED; }
+    const size_t o_qcounts = take(sizeof(int32_t) * ((size_t)ix->n_quads + 1));
+    const size_t o_quad_ptr = take(sizeof(int32_t) * ((size_t)ix->n_quads + 1));
+    const size_t o_quad_tiles = take(sizeof(int32_t) * (size_t)(ix->cap_quad_tiles + 1));
+    const size_t o_quad_meta = take(sizeof(int32_t) * 2);
 
     static bool pool_ready[LVSA_MAX_DEVICES] = {};
     if (!pool_ready[ix->device]) {
@@ -326,6 +394,8 @@ lvsa_status_t lvsa_index_build_device(lvsa_index *ix, cudaStream_t stream) {
     ix->d_item_ptr = (int32_t *)(a + o_item_ptr); ix->d_item_tiles = (int32_t *)(a + o_item_tiles);
     ix->d_item_col0 = (int32_t *)(a + o_item_col0);
     ix->d_kept_cols = (unsigned long long *)(a + o_kept_cols);
+    int32_t *d_qcounts = (int32_t *)(a + o_qcounts), *d_quad_meta = (int32_t *)(a + o_quad_meta);
+    ix->d_quad_ptr = (int32_t *)(a + o_quad_ptr); ix->d_quad_tiles = (int32_t *)(a + o_quad_tiles);
 
     LVSA_CUDA_TRY(cudaMemsetAsync(ix->d_meta, 0, sizeof(int32_t) * 8, stream));
     LVSA_CUDA_TRY(cudaMemsetAsync(ix->d_kept_cols, 0, sizeof(unsigned long long), stream));
@@ -346,6 +416,16 @@ lvsa_status_t lvsa_index_build_device(lvsa_index *ix, cudaStream_t stream) {
         (long long)ix->N, p.P, T, ix->Tf, p.tile_q, p.tile_k, ix->nq, ix->nk, words, ix->d_abits, ix->d_indptr,
         ix->d_item_ptr, nullptr, nullptr, ix->d_indices, ix->d_flags, ix->d_item_tiles, ix->d_item_col0, ix->d_meta,
         ix->d_kept_cols);
+    if (quads) {
+        const int nqd = (int)ix->n_quads;
+        lvsa_quads_kernel<false><<<nqd, 256, 0, stream>>>((long long)ix->N, p.P, ix->Tf, p.tile_q, p.tile_k, ix->nq, ix->nk,
+                                                          words, ix->d_abits, nullptr, d_qcounts, nullptr, ix->d_meta);
+        // block 0 scans the quad counts (total -> quad_meta[0]); block 1 has nothing to do
+        lvsa_scan_kernel<<<2, 1024, 0, stream>>>(d_qcounts, nqd, ix->d_quad_ptr, d_quad_meta, (long long)ix->cap_quad_tiles,
+                                                 d_qcounts, 0, d_qcounts + nqd, d_quad_meta + 1, 1ll << 40, ix->d_meta + 7);
+        lvsa_quads_kernel<true><<<nqd, 256, 0, stream>>>((long long)ix->N, p.P, ix->Tf, p.tile_q, p.tile_k, ix->nq, ix->nk,
+                                                         words, ix->d_abits, ix->d_quad_ptr, nullptr, ix->d_quad_tiles, ix->d_meta);
+    }
     LVSA_CUDA_TRY(cudaGetLastError());
     ix->meta_fetched = false;
     return LVSA_OK;

@@ -18,6 +18,10 @@ constexpr int LVSA_ST_SKIP = 0, LVSA_ST_FULL = 1, LVSA_ST_PARTIAL = 2;
 constexpr int LVSA_ITEM_J_BITS = 26;
 constexpr int LVSA_ITEM_J_MASK = (1 << LVSA_ITEM_J_BITS) - 1;
 constexpr int LVSA_ITEM_W_SHIFT = 30;
+// Work-list entry of the 4-CTA-cluster kernel: bits [0,24): kv tile j; bits [24 + 2w, 26 + 2w): state
+// of the quad's q tile w (w = 0..3).
+constexpr int LVSA_QUAD_J_BITS = 24;
+constexpr int LVSA_QUAD_J_MASK = (1 << LVSA_QUAD_J_BITS) - 1;
 
 // Geometry of kv tile j under either tiling (include/lvsa.h, readings R14 / R25): first token, valid
 // width, and the frame row of its first token.  T = video frames, Tf = T + (text pseudo-frame).
@@ -80,6 +84,9 @@ struct lvsa_index {
     int32_t *d_item_ptr = nullptr;    // [n_items+1]
     int32_t *d_item_tiles = nullptr;  // [n_item_tiles], encoding above
     int32_t *d_item_col0 = nullptr;   // [n_item_tiles], first token of the entry's kv tile
+    int64_t n_quads = 0, cap_quad_tiles = 0;   // LVSA_KERNEL_TCGEN05_QUAD only
+    int32_t *d_quad_ptr = nullptr;    // [n_quads+1]
+    int32_t *d_quad_tiles = nullptr;  // entries as above
     mutable int64_t kept_cols = 0;    // sum of computed kv columns over the kept pairs
     unsigned long long *d_kept_cols = nullptr;
 };
@@ -123,6 +130,7 @@ lvsa_status_t lvsa_attn_sm100_pair_launch_heads(const lvsa_index *ix, const void
                                                 const void *v, void *out, float *lse, int h0, int hc,
                                                 cudaStream_t stream);
 lvsa_status_t lvsa_attn_sm100_pair_prepare(int device);
+int lvsa_attn_sm100_pair_grid(const lvsa_index *ix, int hc);   // CTAs of a launch over hc heads (after prepare)
 int lvsa_attn_uses_pair_kernel(const lvsa_index *ix);   // lvsa_attn_sm100.cu
 
 // lvsa_capi.cu: one-time kernel setup for the index's kernel (used by the schedule driver)

@@ -321,10 +321,22 @@ __device__ __forceinline__ void umma_ts_pair(uint32_t d_tmem, uint32_t a_tmem, u
 }
 // Arrive on the mbarrier at this shared-memory offset in BOTH CTAs of the pair once every MMA issued
 // so far by this thread has completed.
-__device__ __forceinline__ void umma_commit_pair(uint32_t bar) {
+// `cta_mask`: cluster ranks whose barrier (same offset) receives the arrival.
+__device__ __forceinline__ void umma_commit_pair(uint32_t bar, uint16_t cta_mask = 3) {
     asm volatile(
         "tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
-        ::"r"(bar), "h"((uint16_t)3)
+        ::"r"(bar), "h"(cta_mask)
+        : "memory");
+}
+// cta_group::2 tiled load MULTICAST to the CTAs of `cta_mask` (same shared-memory offset in each).
+// `bar_rel` is the issuing CTA's own barrier address with the peer bit (bit 24) cleared: every
+// destination CTA then counts its bytes on that barrier in the LEADER of its own pair.
+__device__ __forceinline__ void tma_load_4d_pair_mc(uint32_t dst, const CUtensorMap *m, uint32_t bar_rel, uint16_t cta_mask,
+                                                    int c0, int c1, int c2, int c3) {
+    asm volatile(
+        "cp.async.bulk.tensor.4d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes.multicast::cluster "
+        "[%0], [%1, {%4, %5, %6, %7}], [%2], %3;"
+        ::"r"(dst), "l"(reinterpret_cast<uint64_t>(m)), "r"(bar_rel), "h"(cta_mask), "r"(c0), "r"(c1), "r"(c2), "r"(c3)
         : "memory");
 }
 // 4-D tiled load into this CTA's shared memory; completion bytes are counted on the mbarrier at
