@@ -134,7 +134,8 @@ def run_ours(args):
     stream = torch.cuda.current_stream()
     steps_cycle = list(w.steps) if w.steps else [0]
 
-    kernel_of = {"default": binding.KERNEL_AUTO, "quad": binding.KERNEL_TCGEN05_QUAD, "v0": binding.KERNEL_TCGEN05_V0}
+    kernel_of = {"default": binding.KERNEL_AUTO, "quad": binding.KERNEL_TCGEN05_QUAD, "hybrid": binding.KERNEL_TCGEN05_HYBRID,
+                 "v0": binding.KERNEL_TCGEN05_V0}
 
     def build(s, **kw):
         kw.setdefault("kernel", kernel_of[args.kernel])
@@ -524,7 +525,7 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-dense", action="store_true")
     ap.add_argument("--no-schedule", action="store_true")
-    ap.add_argument("--kernel", default="default", choices=["default", "quad", "v0"],
+    ap.add_argument("--kernel", default="default", choices=["default", "quad", "hybrid", "v0"],
                     help="attention kernel of the timed steps (default: the CTA-pair kernel); for A/B runs and ncu captures")
     ap.add_argument("--window", type=int, default=None, help="override W of the workload (sensitivity runs)")
     ap.add_argument("--anchors", type=int, default=None, help="override a = C - (2W+1) of the workload")

@@ -44,9 +44,12 @@ enum { LVSA_DTYPE_BF16 = 0, LVSA_DTYPE_FP32 = 1 };             /* element type o
  * as an A/B and cross-check variant; same results within the stated tolerance).
  * LVSA_KERNEL_TCGEN05_QUAD (d = 128, token-0 kv tiles): the CTA-pair kernel run as clusters of FOUR CTAs,
  * two MMA pairs working on adjacent work items that receive every K/V tile from ONE TMA load
- * (multicast), which halves the L2 -> SM traffic. */
+ * (multicast), which halves the L2 -> SM traffic.
+ * LVSA_KERNEL_TCGEN05_HYBRID: 4-CTA clusters on the SMs they can cover (a cluster needs four SMs of one GPC:
+ * 132 of 148 on B200) and CTA pairs on the rest, as two launches side by side on the caller's stream and an
+ * internal one (forked and joined with events; capturable). */
 enum { LVSA_KERNEL_AUTO = 0, LVSA_KERNEL_SIMT = 1, LVSA_KERNEL_TCGEN05 = 2, LVSA_KERNEL_TCGEN05_V0 = 3,
-       LVSA_KERNEL_TCGEN05_QUAD = 4 };
+       LVSA_KERNEL_TCGEN05_QUAD = 4, LVSA_KERNEL_TCGEN05_HYBRID = 5 };
 /* Memory order of q, k, v, out (PAPER.md:31 fixes only N = T*P, not the order of the axes):
  * NHD = [B, N, H, d] (default), HND = [B, H, N, d]; d is always fastest.  lse is [B, H, N] in both. */
 enum { LVSA_LAYOUT_NHD = 0, LVSA_LAYOUT_HND = 1 };

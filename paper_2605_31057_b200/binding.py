@@ -20,7 +20,7 @@ ALL_TILES = -1
 TILE_FULL, TILE_PARTIAL = 0, 1
 TIE_LO, TIE_HI = 0, 1
 DTYPE_BF16, DTYPE_FP32 = 0, 1
-KERNEL_AUTO, KERNEL_SIMT, KERNEL_TCGEN05, KERNEL_TCGEN05_V0, KERNEL_TCGEN05_QUAD = 0, 1, 2, 3, 4
+KERNEL_AUTO, KERNEL_SIMT, KERNEL_TCGEN05, KERNEL_TCGEN05_V0, KERNEL_TCGEN05_QUAD, KERNEL_TCGEN05_HYBRID = 0, 1, 2, 3, 4, 5
 LAYOUT_NHD, LAYOUT_HND = 0, 1
 KV_TILES_TOKEN0, KV_TILES_FRAME_ALIGNED = 0, 1
 KV_PAD = 32

@@ -26,6 +26,8 @@
 #include <cuda.h>
 #include <cuda_bf16.h>
 
+#include <mutex>
+
 #include "lvsa_internal.h"
 #include "sm100_ptx.cuh"
 #include "lvsa_softmax.cuh"
@@ -99,7 +101,7 @@ lvsa_attn_sm100_pair_kernel(const __grid_constant__ CUtensorMap tmap_q,
                             const int32_t *__restrict__ item_ptr, const int32_t *__restrict__ item_tiles,
                             const int32_t *__restrict__ item_col0,
                             const uint32_t *__restrict__ a_bits, int words, long long N, int P, int T,
-                            int H, int h0, int hc, int n_items, long long n_work, float scale_log2) {
+                            int H, int h0, int hc, int n_items, long long work0, long long n_work, float scale_log2) {
     using SM = SmemP<NS>;
     constexpr bool VARW = MODE == MODE_VARW, QUAD = MODE == MODE_QUAD;
     constexpr int CL = QUAD ? 4 : 2;                   // CTAs per cluster
@@ -171,7 +173,7 @@ lvsa_attn_sm100_pair_kernel(const __grid_constant__ CUtensorMap tmap_q,
         if (w == 1) tok_pass();     // the first token: tile 0 belongs to warpgroup 0
         uint32_t tc = 0;            // kv tiles of this CTA so far (all items); tile tc belongs to warpgroup tc & 1
         uint32_t oc = 0;            // items finished
-        for (long long work = pair; work < n_work; work += n_pairs) {
+        for (long long work = work0 + pair; work < n_work; work += n_pairs) {   // works [work0, n_work) of this launch
             const int item = (int)(work % n_items);
             const int bh = (int)(work / n_items), h = h0 + bh % hc, b = bh / hc;   // heads [h0, h0 + hc) of H
             const long long my_row = unit_row0(item) + rw;
@@ -445,7 +447,7 @@ lvsa_attn_sm100_pair_kernel(const __grid_constant__ CUtensorMap tmap_q,
                 }
                 ++kv_it;
             };
-            for (long long work = pair; work < n_work; work += n_pairs) {
+            for (long long work = work0 + pair; work < n_work; work += n_pairs) {   // works [work0, n_work) of this launch
                 const int item = (int)(work % n_items);
                 const int bh = (int)(work / n_items), h = h0 + bh % hc, b = bh / hc;   // heads [h0, h0 + hc) of H
                 const long long row0 = unit_row0(item);
@@ -518,7 +520,7 @@ lvsa_attn_sm100_pair_kernel(const __grid_constant__ CUtensorMap tmap_q,
                 ++kv_it;
                 mbar_wait(bar(SM::KV_FULL + stage), n & 1u);
             };
-            for (long long work = pair; work < n_work; work += n_pairs) {
+            for (long long work = work0 + pair; work < n_work; work += n_pairs) {   // works [work0, n_work) of this launch
                 const int item = (int)(work % n_items);
                 const int e0 = __shfl_sync(0xffffffffu, __ldg(item_ptr + item), 0);
                 const int e1 = __shfl_sync(0xffffffffu, __ldg(item_ptr + item + 1), 0);
@@ -622,15 +624,28 @@ lvsa_status_t lvsa_attn_sm100_pair_prepare(int device) {
     return LVSA_OK;
 }
 
+// HYBRID (LVSA_KERNEL_TCGEN05_HYBRID): 4-CTA clusters on the SMs they can cover, CTA pairs on the rest,
+// as two launches that run side by side (the second on an internal stream, forked from and joined back to
+// the caller's stream with events, which also works under stream capture).  The work is split statically
+// at a quad boundary in proportion to the SMs of the two parts.
+struct HybridSide { cudaStream_t side = nullptr; cudaEvent_t fork = nullptr, join = nullptr; };
+static HybridSide g_hybrid[LVSA_MAX_DEVICES];
+static std::mutex g_hybrid_mutex;
+#ifndef LVSA_HYBRID_QUAD_SPEED
+#define LVSA_HYBRID_QUAD_SPEED 1.04   // measured: work per SM and second of the 4-CTA clusters relative to the pairs
+#endif
+
+static bool is_quad(const lvsa_index *ix) { return ix->p.kernel == LVSA_KERNEL_TCGEN05_QUAD || ix->p.kernel == LVSA_KERNEL_TCGEN05_HYBRID; }
+
 int lvsa_attn_sm100_pair_grid(const lvsa_index *ix, int hc) {
-    const bool quad = ix->p.kernel == LVSA_KERNEL_TCGEN05_QUAD;
+    if (ix->p.kernel == LVSA_KERNEL_TCGEN05_HYBRID) return g_pair_n_sm[ix->device] / 2 * 2;   // both parts together
+    const bool quad = is_quad(ix);
     const int cl = quad ? 4 : 2;
     const long long n_work = (quad ? ix->n_quads : ix->n_items) * hc * ix->p.B;
     long long n_clusters = quad ? g_quad_clusters[ix->device] : g_pair_n_sm[ix->device] / cl;
     if (n_work < n_clusters) n_clusters = n_work;
     return (int)(cl * n_clusters);
 }
-
 // Heads [h0, h0 + hc) only (all batches): the host entry point pipelines head groups against the
 // PCIe copies.  q, k, v, out, lse are the FULL tensors.
 lvsa_status_t lvsa_attn_sm100_pair_launch_heads(const lvsa_index *ix, const void *q, const void *k, const void *v,
@@ -644,19 +659,50 @@ lvsa_status_t lvsa_attn_sm100_pair_launch_heads(const lvsa_index *ix, const void
     if ((st = lvsa_make_tmap_bf16(&mv, v, ix, BT)) != LVSA_OK) return st;
     if ((st = lvsa_make_tmap_bf16(&mo, out, ix, 128)) != LVSA_OK) return st;
     if ((st = lvsa_attn_sm100_pair_prepare(ix->device)) != LVSA_OK) return st;
-    const bool quad = ix->p.kernel == LVSA_KERNEL_TCGEN05_QUAD;
-    const int cl = quad ? 4 : 2;                                             // CTAs per cluster
-    const long long n_units = quad ? ix->n_quads : ix->n_items;             // work units per (head, batch)
-    const long long n_work = n_units * hc * ix->p.B;
-    const long long n_clusters = lvsa_attn_sm100_pair_grid(ix, hc) / cl;
     const float scale_log2 = ix->p.softmax_scale * 1.4426950408889634f;
-    auto kern = quad ? lvsa_attn_sm100_pair_kernel<NS, MODE_QUAD>
-              : ix->p.kv_tiling == LVSA_KV_TILES_FRAME_ALIGNED ? lvsa_attn_sm100_pair_kernel<NS, MODE_VARW>
-                                                               : lvsa_attn_sm100_pair_kernel<NS, MODE_TOKEN0>;
-    kern<<<(unsigned)(cl * n_clusters), NTHREADS, SM::BYTES, stream>>>(
-        mq, mk, mv, mo, lse, quad ? ix->d_quad_ptr : ix->d_item_ptr, quad ? ix->d_quad_tiles : ix->d_item_tiles,
-        ix->d_item_col0, ix->d_abits, ix->words,
-        (long long)ix->N, ix->p.P, ix->Tf, ix->p.H, h0, hc, (int)n_units, n_work, scale_log2);
+    // one launch over the works [work0, work_end) of its kind (quads for MODE_QUAD, items otherwise)
+    auto launch = [&](int mode, long long work0, long long work_end, long long n_clusters, cudaStream_t s) {
+        if (work_end <= work0) return;
+        if (work_end - work0 < n_clusters) n_clusters = work_end - work0;
+        const bool quad = mode == MODE_QUAD;
+        auto kern = quad ? lvsa_attn_sm100_pair_kernel<NS, MODE_QUAD>
+                  : mode == MODE_VARW ? lvsa_attn_sm100_pair_kernel<NS, MODE_VARW> : lvsa_attn_sm100_pair_kernel<NS, MODE_TOKEN0>;
+        kern<<<(unsigned)((quad ? 4 : 2) * n_clusters), NTHREADS, SM::BYTES, s>>>(
+            mq, mk, mv, mo, lse, quad ? ix->d_quad_ptr : ix->d_item_ptr, quad ? ix->d_quad_tiles : ix->d_item_tiles,
+            ix->d_item_col0, ix->d_abits, ix->words, (long long)ix->N, ix->p.P, ix->Tf, ix->p.H, h0, hc,
+            (int)(quad ? ix->n_quads : ix->n_items), work0, work_end, scale_log2);
+    };
+    const int dev = ix->device;
+    const long long item_works = ix->n_items * hc * ix->p.B, quad_works = ix->n_quads * hc * ix->p.B;
+    if (ix->p.kernel == LVSA_KERNEL_TCGEN05_HYBRID) {
+        const long long nqc = g_quad_clusters[dev], pairs_left = (g_pair_n_sm[dev] - 4 * nqc) / 2;
+        // the pairs' share of the quads, rounded to whole quads; the pair launch starts at the first item of quad wq1
+        const double share = pairs_left <= 0 ? 0.0 : 2.0 * pairs_left / (4.0 * nqc * LVSA_HYBRID_QUAD_SPEED + 2.0 * pairs_left);
+        long long wq1 = quad_works - (long long)(quad_works * share + 0.5);
+        if (wq1 < 0) wq1 = 0;
+        const long long item0 = (wq1 / ix->n_quads) * ix->n_items + 2 * (wq1 % ix->n_quads);
+        if (wq1 == quad_works || item0 >= item_works) {
+            launch(MODE_QUAD, 0, quad_works, nqc, stream);
+        } else {
+            std::lock_guard<std::mutex> lock(g_hybrid_mutex);
+            HybridSide &hs = g_hybrid[dev];
+            if (hs.side == nullptr) {
+                LVSA_CUDA_TRY(cudaStreamCreateWithFlags(&hs.side, cudaStreamNonBlocking));
+                LVSA_CUDA_TRY(cudaEventCreateWithFlags(&hs.fork, cudaEventDisableTiming));
+                LVSA_CUDA_TRY(cudaEventCreateWithFlags(&hs.join, cudaEventDisableTiming));
+            }
+            LVSA_CUDA_TRY(cudaEventRecord(hs.fork, stream));
+            LVSA_CUDA_TRY(cudaStreamWaitEvent(hs.side, hs.fork, 0));
+            launch(MODE_QUAD, 0, wq1, nqc, stream);                      // first: the clusters need whole GPC quarters
+            launch(MODE_TOKEN0, item0, item_works, pairs_left, hs.side);
+            LVSA_CUDA_TRY(cudaEventRecord(hs.join, hs.side));
+            LVSA_CUDA_TRY(cudaStreamWaitEvent(stream, hs.join, 0));
+        }
+    } else if (ix->p.kernel == LVSA_KERNEL_TCGEN05_QUAD) {
+        launch(MODE_QUAD, 0, quad_works, g_quad_clusters[dev], stream);
+    } else {
+        launch(ix->p.kv_tiling == LVSA_KV_TILES_FRAME_ALIGNED ? MODE_VARW : MODE_TOKEN0, 0, item_works, g_pair_n_sm[dev] / 2, stream);
+    }
     LVSA_CUDA_TRY(cudaGetLastError());
     return LVSA_OK;
 }

@@ -58,7 +58,7 @@ static size_t elem_size(const lvsa_index *ix) { return ix->p.dtype == LVSA_DTYPE
 static int use_tcgen05(const lvsa_index *ix) {
     if (ix->p.kernel == LVSA_KERNEL_SIMT) return 0;
     if (ix->p.kernel == LVSA_KERNEL_TCGEN05 || ix->p.kernel == LVSA_KERNEL_TCGEN05_V0 ||
-        ix->p.kernel == LVSA_KERNEL_TCGEN05_QUAD) return 1;
+        ix->p.kernel == LVSA_KERNEL_TCGEN05_QUAD || ix->p.kernel == LVSA_KERNEL_TCGEN05_HYBRID) return 1;
     return ix->p.dtype == LVSA_DTYPE_BF16;
 }
 
@@ -91,7 +91,7 @@ lvsa_status_t lvsa_build_block_index_ex(const lvsa_params_t *params, void *strea
     if (p.n_text < 0) { lvsa_set_error("n_text must be >= 0"); return LVSA_EINVAL; }
     if (p.tie_break != LVSA_TIE_LO && p.tie_break != LVSA_TIE_HI) { lvsa_set_error("bad tie_break"); return LVSA_EINVAL; }
     if (p.dtype != LVSA_DTYPE_BF16 && p.dtype != LVSA_DTYPE_FP32) { lvsa_set_error("bad dtype"); return LVSA_EINVAL; }
-    if (p.kernel < LVSA_KERNEL_AUTO || p.kernel > LVSA_KERNEL_TCGEN05_QUAD) { lvsa_set_error("bad kernel"); return LVSA_EINVAL; }
+    if (p.kernel < LVSA_KERNEL_AUTO || p.kernel > LVSA_KERNEL_TCGEN05_HYBRID) { lvsa_set_error("bad kernel"); return LVSA_EINVAL; }
     if (p.layout != LVSA_LAYOUT_NHD && p.layout != LVSA_LAYOUT_HND) { lvsa_set_error("bad layout"); return LVSA_EINVAL; }
     if (p.host_groups < 0) { lvsa_set_error("host_groups must be >= 0"); return LVSA_EINVAL; }
     if (p.kv_tiling != LVSA_KV_TILES_TOKEN0 && p.kv_tiling != LVSA_KV_TILES_FRAME_ALIGNED) { lvsa_set_error("bad kv_tiling"); return LVSA_EINVAL; }
@@ -103,12 +103,12 @@ lvsa_status_t lvsa_build_block_index_ex(const lvsa_params_t *params, void *strea
         lvsa_set_error("tiles must be 128x128 for d = 128 and 64x64 for d = 64");
         return LVSA_EUNSUPPORTED;
     }
-    if (p.kernel == LVSA_KERNEL_TCGEN05_QUAD && (p.d != 128 || p.kv_tiling != LVSA_KV_TILES_TOKEN0)) {
+    if ((p.kernel == LVSA_KERNEL_TCGEN05_QUAD || p.kernel == LVSA_KERNEL_TCGEN05_HYBRID) && (p.d != 128 || p.kv_tiling != LVSA_KV_TILES_TOKEN0)) {
         lvsa_set_error("the 4-CTA-cluster kernel takes d = 128 and token-0 kv tiles only");
         return LVSA_EUNSUPPORTED;
     }
     if (p.dtype == LVSA_DTYPE_FP32 && (p.kernel == LVSA_KERNEL_TCGEN05 || p.kernel == LVSA_KERNEL_TCGEN05_V0 ||
-                                       p.kernel == LVSA_KERNEL_TCGEN05_QUAD)) {
+                                       p.kernel == LVSA_KERNEL_TCGEN05_QUAD || p.kernel == LVSA_KERNEL_TCGEN05_HYBRID)) {
         lvsa_set_error("the tcgen05 kernel takes bf16 only");
         return LVSA_EUNSUPPORTED;
     }
@@ -345,7 +345,7 @@ lvsa_status_t lvsa_index_info(const lvsa_index_t *ix, lvsa_index_info_t *info) {
     info->initial_anchors = p.initial_anchors; info->layout = p.layout; info->kv_tiling = p.kv_tiling;
     info->kept_cols = ix->kept_cols;
     info->kernel = !use_tcgen05(ix) ? LVSA_KERNEL_SIMT
-                 : (p.kernel == LVSA_KERNEL_TCGEN05_V0 || p.kernel == LVSA_KERNEL_TCGEN05_QUAD ? p.kernel : LVSA_KERNEL_TCGEN05);
+                 : (p.kernel == LVSA_KERNEL_TCGEN05_V0 || p.kernel == LVSA_KERNEL_TCGEN05_QUAD || p.kernel == LVSA_KERNEL_TCGEN05_HYBRID ? p.kernel : LVSA_KERNEL_TCGEN05);
     info->N = ix->N; info->nnz = ix->nnz; info->n_partial = ix->n_partial;
     info->n_items = ix->n_items; info->n_item_tiles = ix->n_item_tiles;
     return LVSA_OK;

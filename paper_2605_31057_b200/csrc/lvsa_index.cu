@@ -363,7 +363,7 @@ lvsa_status_t lvsa_index_build_device(lvsa_index *ix, cudaStream_t stream) {
     const size_t o_item_col0 = take(sizeof(int32_t) * (size_t)(ix->cap_item_tiles + 1));
     const size_t o_kept_cols = take(sizeof(unsigned long long));
     // work lists of the 4-CTA-cluster kernel, built only when that kernel was asked for
-    const bool quads = p.kernel == LVSA_KERNEL_TCGEN05_QUAD;
+    const bool quads = p.kernel == LVSA_KERNEL_TCGEN05_QUAD || p.kernel == LVSA_KERNEL_TCGEN05_HYBRID;
     ix->n_quads = quads ? (ix->nq + 3) / 4 : 0;
     long long per_quad = per_q * 4; if (per_quad > ix->nk) per_quad = ix->nk;
     ix->cap_quad_tiles = quads ? per_quad * ix->n_quads + text_q * ix->nk : 0;

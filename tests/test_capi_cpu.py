@@ -31,7 +31,7 @@ def test_header_constants_match_binding():
     """The enum values the binding hard-codes are the header's."""
     src = open(os.path.join(ROOT, "include", "lvsa.h")).read()
     vals = {k: int(v) for k, v in re.findall(r"\b(LVSA_[A-Z0-9_]+)\s*=\s*(-?\d+)", src)}
-    for name in ("KERNEL_AUTO", "KERNEL_SIMT", "KERNEL_TCGEN05", "KERNEL_TCGEN05_V0", "KERNEL_TCGEN05_QUAD", "LAYOUT_NHD", "LAYOUT_HND",
+    for name in ("KERNEL_AUTO", "KERNEL_SIMT", "KERNEL_TCGEN05", "KERNEL_TCGEN05_V0", "KERNEL_TCGEN05_QUAD", "KERNEL_TCGEN05_HYBRID", "LAYOUT_NHD", "LAYOUT_HND",
                  "KV_TILES_TOKEN0", "KV_TILES_FRAME_ALIGNED",
                  "DTYPE_BF16", "DTYPE_FP32", "TIE_LO", "TIE_HI", "TILE_FULL", "TILE_PARTIAL", "OK", "EINVAL",
                  "EUNSUPPORTED", "ECUDA", "ENOMEM"):
@@ -58,7 +58,7 @@ def test_argument_validation_needs_no_gpu():
            dict(T=4, P=4, H=1, d=64, layer=-1), dict(T=1 << 16, P=1 << 16, H=1, d=64),
            dict(T=4, P=4, H=1, d=64, tie_break=7), dict(T=4, P=4, H=1, d=64, initial_anchors=-1),
            dict(T=4, P=4, H=1, d=64, n_text=-1), dict(T=4, P=4, H=1, d=64, layout=2),
-           dict(T=4, P=4, H=1, d=64, kernel=5), dict(T=4, P=4, H=1, d=64, host_groups=-1),
+           dict(T=4, P=4, H=1, d=64, kernel=6), dict(T=4, P=4, H=1, d=64, host_groups=-1),
            dict(T=4, P=4, H=1, d=64, kv_tiling=2)]
     for kw in bad:
         with pytest.raises(binding.LvsaError) as ei:

@@ -1,7 +1,8 @@
-"""GPU parity for the 4-CTA-cluster variant of the attention kernel (LVSA_KERNEL_TCGEN05_QUAD, SURVEY.md
-section 8f row f4: K/V tiles shared by two MMA pairs through one multicast TMA load), through the C ABI,
-against the fp64 oracle element by element.  The index (CSR) is the same as for the other kernels; the
-variant only consumes a different work list (unions over four q tiles)."""
+"""GPU parity for the 4-CTA-cluster variants of the attention kernel (K/V tiles
+shared by two MMA pairs through one multicast TMA load), through the C ABI, against the fp64 oracle element
+by element: LVSA_KERNEL_TCGEN05_QUAD (clusters of four only) and LVSA_KERNEL_TCGEN05_HYBRID (clusters of four
+plus CTA pairs on the SMs the clusters cannot cover, two launches side by side).  The index (CSR) is the same
+as for the other kernels; the variants only consume a different work list (unions over four q tiles)."""
 import numpy as np
 import pytest
 import torch
@@ -11,11 +12,13 @@ from paper_2605_31057_b200 import binding, inputs
 
 pytestmark = pytest.mark.gpu
 
-QUAD = dict(dtype=binding.DTYPE_BF16, kernel=binding.KERNEL_TCGEN05_QUAD)
+KERNELS = {"quad": dict(dtype=binding.DTYPE_BF16, kernel=binding.KERNEL_TCGEN05_QUAD),
+           "hybrid": dict(dtype=binding.DTYPE_BF16, kernel=binding.KERNEL_TCGEN05_HYBRID)}
+QUAD = KERNELS["quad"]
 W = inputs.Workload
 
 
-def run_case(w, steps, rows=None, seed=None, anchors=None, hnd=False):
+def run_case(w, steps, rows=None, seed=None, anchors=None, hnd=False, QUAD=QUAD):
     q, k, v = inputs.make_qkv(w, "cuda", torch.bfloat16, seed=seed)
     rows = np.arange(w.N) if rows is None else rows
     for s in steps:
@@ -26,7 +29,7 @@ def run_case(w, steps, rows=None, seed=None, anchors=None, hnd=False):
         else:
             ix = build_index(w, s, anchors=anchors, **QUAD)
             out, lse = gpu_attn(w, ix, q, k, v)
-        assert ix.info().kernel == binding.KERNEL_TCGEN05_QUAD
+        assert ix.info().kernel == QUAD["kernel"]
         for b in range(w.B):
             ref, ref_lse = oracle_attn(w, q, k, v, s, rows, anchors=anchors, b=b)
             st = compare(out, lse, ref, ref_lse, rows, b)
@@ -36,14 +39,16 @@ def run_case(w, steps, rows=None, seed=None, anchors=None, hnd=False):
         ix.destroy()
 
 
+@pytest.mark.parametrize("kname", list(KERNELS))
 @pytest.mark.parametrize("name", ["small128", "small128_text", "small128_k0"])
-def test_all_rows(name):
+def test_all_rows(name, kname):
     w = inputs.WORKLOADS[name]
-    run_case(w, w.steps[:3])
-    run_case(w, w.steps[:1], hnd=True)
+    run_case(w, w.steps[:3], QUAD=KERNELS[kname])
+    run_case(w, w.steps[:1], hnd=True, QUAD=KERNELS[kname])
 
 
-def test_edge_shapes():
+@pytest.mark.parametrize("kname", list(KERNELS))
+def test_edge_shapes(kname):
     cases = [W("one_tile", 1, T=1, P=128, H=2, d=128, tile=128, W=0, a=0),           # one q tile: three of four CTAs have no rows
              W("two_tiles", 1, T=2, P=128, H=1, d=128, tile=128, W=0, a=1),
              W("odd_nq", 1, T=3, P=128, H=1, d=128, tile=128, W=0, a=1),             # nq = 3
@@ -52,17 +57,18 @@ def test_edge_shapes():
              W("dense_window", 1, T=5, P=90, H=2, d=128, tile=128, W=2, a=0),        # 2W+1 >= T: Eq. 1
              W("many_heads", 1, T=4, P=200, H=9, d=128, tile=128, W=1, a=1)]
     for w in cases:
-        run_case(w, (0, 1))
-    run_case(cases[4], (0,), anchors=binding.ALL_TILES)
+        run_case(w, (0, 1), QUAD=KERNELS[kname])
+    run_case(cases[4], (0,), anchors=binding.ALL_TILES, QUAD=KERNELS[kname])
 
 
-def test_seeded_shape_sweep():
+@pytest.mark.parametrize("kname", list(KERNELS))
+def test_seeded_shape_sweep(kname):
     rng = np.random.default_rng(20260602)
     for case in range(20):
         w = W(f"quad_sweep{case}", 1, T=int(rng.integers(1, 14)), P=int(rng.integers(17, 420)), H=int(rng.integers(1, 4)),
               d=128, tile=128, W=int(rng.integers(0, 3)), a=int(rng.choice([0, 1, 2, 3, 5, binding.ALL_TILES])),
               B=int(rng.integers(1, 3)), n_text=int(rng.choice([0, 0, 1, 64, 150])), k0=int(rng.choice([0, 0, 1, 2])))
-        run_case(w, (int(rng.integers(0, 7)),), seed=3000 + case)
+        run_case(w, (int(rng.integers(0, 7)),), seed=3000 + case, QUAD=KERNELS[kname])
 
 
 def test_structured_logits_growing_maximum():
@@ -93,6 +99,19 @@ def test_grid_and_repeatability_and_host_entry_point():
     sms = torch.cuda.get_device_properties(0).multi_processor_count
     assert ixp.grid() == sms // 2 * 2                                  # CTA pairs: every SM
     assert 0 < ix.grid() <= sms and ix.grid() % 4 == 0                 # resident 4-CTA clusters only
+    ixh = build_index(w, w.steps[0], **KERNELS["hybrid"])
+    assert ixh.grid() == sms // 2 * 2                                  # clusters of four + pairs: every SM
+    hyb, hyb_lse = gpu_attn(w, ixh, q, k, v)
+    # CUDA-graph capture of the two side-by-side launches (fork / join with events on an internal stream)
+    g, side, out_g = torch.cuda.CUDAGraph(), torch.cuda.Stream(), torch.zeros_like(q)
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        with torch.cuda.graph(g, stream=side):
+            binding.lvsa_attn_fwd(q, k, v, ixh, out_g, None, stream=side.cuda_stream)
+    torch.cuda.current_stream().wait_stream(side)
+    g.replay(); torch.cuda.synchronize()
+    assert torch.equal(out_g, hyb)
+    ixh.destroy()
     ref, ref_lse = gpu_attn(w, ix, q, k, v)
     for _ in range(10):                                                # timing-independent result
         out, lse = gpu_attn(w, ix, q, k, v)
@@ -107,8 +126,9 @@ def test_grid_and_repeatability_and_host_entry_point():
 
 
 @pytest.mark.slow
+@pytest.mark.parametrize("kname", list(KERNELS))
 @pytest.mark.parametrize("name", ["wan1.3b_6x", "hv1.5_2x"])
-def test_large_configs_sampled_rows(name):
+def test_large_configs_sampled_rows(name, kname):
     w = inputs.WORKLOADS[name]
     rows = inputs.sample_rows(w, n_uniform=768, n_edge=256)
-    run_case(w, w.steps[:1], rows=rows)
+    run_case(w, w.steps[:1], rows=rows, QUAD=KERNELS[kname])
