@@ -200,7 +200,9 @@ def run_ours(args):
     step_nnz = [nnz_of[steps_cycle[i % len(steps_cycle)]] for i in range(args.steps)]
     tile_flops = sum(tile_flop(cols_of[steps_cycle[i % len(steps_cycle)]]) for i in range(args.steps))
     nnz_mean = float(np.mean(step_nnz))
-    kern_ms = float(np.mean([a.elapsed_time(b) for a, b in zip(ka, kb)]))     # sustained, inside the step
+    kern_all = [a.elapsed_time(b) for a, b in zip(ka, kb)]
+    kern_ms = float(np.mean(kern_all))                                        # sustained, inside the step
+    kern_median, kern_min = float(np.median(kern_all)), float(np.min(kern_all))
     kern_flops = tile_flops / args.steps
 
     # ---- the same kernel timed alone after an idle gap (burst clocks, no power cap yet): min of 5
@@ -423,6 +425,7 @@ def run_ours(args):
                        "l2": "inputs (3 x %.0f MB) exceed the 126 MB L2; no flush" % (q.numel() * 2 / 1e6),
                        "parallelism": "replicas only (one independent call per GPU)" if world > 1 else "1 GPU"},
             "ms_per_attention_call": round(kern_ms, 4),
+            "ms_per_attention_call_median": round(kern_median, 4), "ms_per_attention_call_min": round(kern_min, 4),
             "tflops_exact_eq2_work": round(useful / (kern_ms * 1e-3) / 1e12, 1),
             "computed_over_exact_work": round(tile_flop(cols_of[steps_cycle[0]]) / useful, 4),
             "index_build_us": round(build_us, 1), "index_build_host_enqueue_us": round(build_host_us, 1),
