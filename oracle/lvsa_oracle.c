@@ -26,7 +26,10 @@
  * adaptive-window frames, dense reduction to library
  * softmax(QK^T/sqrt d)V, per-frame gathered SDPA,
  * rows summing to 1, the Q=0 closed form, token-level N x N brute force on tiny
- * inputs.  Parity UNPINNED (fixed by DESIGN.md readings, not by the paper):
+ * inputs; for the second tile definition (O7b, tests/test_oracle_tiling_fa.py): the
+ * partition properties of the tiling, the same N x N brute force, key-set equality with
+ * negative tests, the reduction to O7 when P is a multiple of Bk, and the kept-column
+ * closed form at the Wan shapes.  Parity UNPINNED (fixed by DESIGN.md readings, not by the paper):
  * the default W (R1), HunyuanVideo's C (R2), the Algorithm-1 tie-break (R5), and the two
  * extension rules the paper names without specifying: dedicated initial anchors (R22,
  * lvsa_oracle_pattern_ex) and text tokens inside self-attention (R23, frame_of;
