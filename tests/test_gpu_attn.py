@@ -149,6 +149,7 @@ def test_closed_form_probe_other_large_configs(name):
 @pytest.mark.slow
 @pytest.mark.parametrize("name,window,anchors", [("hv1.5_2x", 2, 12),      # the exploratory HV budget C = 17
                                                  ("wan1.3b_6x", 1, 18),    # W sweep of profiles/r01e: C = 21 held
+                                                 ("wan1.3b_6x", 3, 14),
                                                  ("wan1.3b_6x", 5, 10)])
 def test_benched_variants_sampled_rows(name, window, anchors):
     """Every configuration that bench.py / profiles/ report a time for is also a checked one: 1024
