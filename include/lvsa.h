@@ -152,6 +152,59 @@ lvsa_status_t lvsa_build_block_index_ex(const lvsa_params_t *params, void *strea
                                         lvsa_index_t **out);
 
 /*
+ * lvsa_build_csr_static — the same block index (steps a1..a5: Alg. 1 :74-89, Eq. 3
+ * :97, Def. 2 :49; token-0 kv tiles, reading R14) for callers that are not allowed to allocate
+ * device memory.
+ *
+ * When to use it.  An inference server commonly gives the whole GPU to one allocator when the model
+ * is loaded (a framework's caching pool, or a fixed memory plan).  Code that runs inside such a
+ * process during the denoising loop (an attention plugin, a step callback) should then not ask the
+ * CUDA driver for memory itself: the request can fail although the pool has room, it stalls the other
+ * streams of the process while it is served, and the memory is invisible to the host's accounting.
+ * lvsa_build_block_index(_ex) allocates an arena per index; THIS call allocates nothing, neither
+ * directly (no cudaMalloc / cudaMallocAsync / cudaFree) nor through a library routine.  The caller
+ * passes the output arrays; the intermediate data of the build (the A(t) bitsets and the per-q-tile
+ * counts) go to a fixed LVSA_STATIC_SCRATCH_BYTES array inside the library image, which every GPU that
+ * loads liblvsa holds until the process exits.
+ *
+ *   params   : as lvsa_build_block_index_ex.  Used: T, P, d, tile_q, tile_k, window, anchors, step,
+ *              tie_break, initial_anchors, n_text.  kv_tiling must be LVSA_KV_TILES_TOKEN0.  The other
+ *              fields (H, B, layer, dtype, kernel, softmax_scale, layout, host_groups) do not change
+ *              the index and are ignored.
+ *   indptr   : DEVICE, int32[nq + 1], nq = ceil((T*P + n_text) / tile_q).  Always written.
+ *   indices  : DEVICE, int32[capacity]: kept kv tiles, ascending within a q tile.
+ *   flags    : DEVICE, uint8[capacity]: LVSA_TILE_FULL / LVSA_TILE_PARTIAL per entry.
+ *   capacity : entries `indices` and `flags` can hold (nq * ceil(N / tile_k) always suffices).
+ *   nnz      : DEVICE, int32[1]: receives the number of kept (q tile, kv tile) pairs.  If it is
+ *              larger than `capacity`, indices and flags were left untouched (indptr is still valid):
+ *              call again with larger arrays.  The host learns this only by reading *nnz.
+ *   stream   : cudaStream_t the four kernels are enqueued on (NULL = default stream).
+ * The caller owns all four arrays; the library keeps no reference.  The call only enqueues and never
+ * synchronises.  The result is bit-identical to lvsa_index_copy_host of an index built from the same
+ * parameters.
+ *
+ * Limits: T + (n_text > 0) <= LVSA_STATIC_MAX_FRAMES and nq <= LVSA_STATIC_MAX_Q_TILES (about 2.1 M
+ * tokens at 128-token tiles; the largest shape of the paper has 1475 q tiles), else LVSA_EUNSUPPORTED
+ * with a message that names the limit; argument errors are LVSA_EINVAL as for the _ex call.  All of
+ * these are checked on the host before anything is enqueued.
+ *
+ * Sharing.  All calls on one device use the same scratch array, and it keeps what the last call left
+ * in it (each call resets the words that must start at zero, on the stream, before using them).  Two
+ * calls whose kernels can overlap on the GPU (different streams with no ordering between them, or two
+ * host threads) race on it and give wrong indices: order them.  The outputs of a finished call do not
+ * depend on the array any more.
+ *
+ * First call.  The first call made on a device (with that device current) looks up the device address
+ * of the array (cudaGetSymbolAddress) and remembers it; make that first call during set-up, outside
+ * any stream capture.  Later calls on that device only launch kernels.
+ */
+#define LVSA_STATIC_MAX_FRAMES 512
+#define LVSA_STATIC_MAX_Q_TILES 16384
+#define LVSA_STATIC_SCRATCH_BYTES (97 * 1024)
+lvsa_status_t lvsa_build_csr_static(const lvsa_params_t *params, void *stream, int32_t *indptr,
+                                    int32_t *indices, uint8_t *flags, int64_t capacity, int32_t *nnz);
+
+/*
  * lvsa_attn_fwd — step a6/a7: Eq. 2 over the kept tiles, exactly (element-level masking on
  * PARTIAL tiles).
  *   q, k, v : DEVICE pointers, contiguous [B, N, H, d] (or [B, H, N, d] when the index was built

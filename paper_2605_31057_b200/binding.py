@@ -55,7 +55,8 @@ class IndexInfo(C.Structure):
 EXPORTS = ("lvsa_build_block_index", "lvsa_build_block_index_ex", "lvsa_attn_fwd",
            "lvsa_attn_fwd_host", "lvsa_index_destroy", "lvsa_index_info", "lvsa_index_copy_host",
            "lvsa_index_copy_kv_tiles", "lvsa_attn_fwd_launches", "lvsa_attn_fwd_grid", "lvsa_workspace_release", "lvsa_schedule_create",
-           "lvsa_schedule_num_phases", "lvsa_schedule_index", "lvsa_schedule_attn_fwd", "lvsa_schedule_destroy", "lvsa_last_error", "lvsa_version")
+           "lvsa_schedule_num_phases", "lvsa_schedule_index", "lvsa_schedule_attn_fwd", "lvsa_schedule_destroy", "lvsa_last_error", "lvsa_version",
+           "lvsa_build_csr_static")
 
 _lib = None
 
@@ -98,6 +99,9 @@ def lib() -> C.CDLL:
         L.lvsa_schedule_attn_fwd.argtypes = [C.c_void_p, C.c_int] + [C.c_void_p] * 6
         L.lvsa_schedule_destroy.restype = None
         L.lvsa_schedule_destroy.argtypes = [C.c_void_p]
+        L.lvsa_build_csr_static.restype = C.c_int
+        L.lvsa_build_csr_static.argtypes = [C.POINTER(Params), C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
+                                            C.c_int64, C.c_void_p]
         L.lvsa_last_error.restype = C.c_char_p
         L.lvsa_version.restype = C.c_char_p
         _lib = L
@@ -203,6 +207,29 @@ def lvsa_build_block_index_ex(stream: int = 0, **kw) -> BlockIndex:
     out = C.c_void_p()
     _check(lib().lvsa_build_block_index_ex(C.byref(p), C.c_void_p(stream), C.byref(out)))
     return BlockIndex(out.value)
+
+
+STATIC_MAX_FRAMES, STATIC_MAX_Q_TILES = 512, 16384
+
+
+def lvsa_build_csr_static(indptr, indices, flags, nnz, stream: int | None = None, **kw) -> None:
+    """The block index written into the caller's CUDA tensors, for callers that must not allocate device
+    memory inside the denoising loop (a plugin in a server whose allocator owns the GPU): indptr int32
+    [nq + 1], indices int32 [capacity], flags uint8 [capacity], nnz int32 [1]; capacity =
+    min(len(indices), len(flags)).  `kw` are lvsa_params_t fields.  Enqueues on `stream` (default: torch's
+    current stream) and returns; read `nnz` to learn whether the list fitted (include/lvsa.h).  Calls
+    that can overlap on the GPU race on the library's fixed scratch array."""
+    p = Params()
+    for k, v in kw.items():
+        if not hasattr(p, k):
+            raise TypeError(f"unknown lvsa_params_t field {k!r}")
+        setattr(p, k, v)
+    if stream is None:
+        import torch
+        stream = torch.cuda.current_stream().cuda_stream
+    cap = min(indices.numel(), flags.numel())
+    _check(lib().lvsa_build_csr_static(C.byref(p), C.c_void_p(stream), _dev_ptr(indptr), _dev_ptr(indices),
+                                       _dev_ptr(flags), C.c_int64(cap), _dev_ptr(nnz)))
 
 
 def _dev_ptr(t) -> C.c_void_p:
