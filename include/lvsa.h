@@ -284,8 +284,14 @@ lvsa_status_t lvsa_index_copy_host(const lvsa_index_t *index, int32_t *indptr, i
  * arithmetic from the parameters; no device work. */
 lvsa_status_t lvsa_index_copy_kv_tiles(const lvsa_index_t *index, int32_t *col0, int32_t *width);
 
-/* Number of kernels lvsa_attn_fwd enqueues per call for this index (bench.py's gpu_launches). */
+/* Number of kernels lvsa_attn_fwd enqueues per call for this index (bench.py's gpu_launches): 1, or 2
+ * for LVSA_KERNEL_TCGEN05_HYBRID when both of its parts get work (needs the index's device current;
+ * -1 on error, 0 on NULL). */
 int lvsa_attn_fwd_launches(const lvsa_index_t *index);
+
+/* Number of kernels the build of this index enqueued: 4 (frames, count, scan, fill), 7 with the work lists
+ * of the 4-CTA-cluster kernels (QUAD / HYBRID); two small memsets come on top. */
+int lvsa_index_build_launches(const lvsa_index_t *index);
 
 /* Number of CTAs the (persistent) tensor-core attention kernel is launched with for this index on its
  * device: 2 x the CTA pairs, or 4 x the 4-CTA clusters that can be resident at once

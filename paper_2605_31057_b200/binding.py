@@ -56,7 +56,7 @@ EXPORTS = ("lvsa_build_block_index", "lvsa_build_block_index_ex", "lvsa_attn_fwd
            "lvsa_attn_fwd_host", "lvsa_index_destroy", "lvsa_index_info", "lvsa_index_copy_host",
            "lvsa_index_copy_kv_tiles", "lvsa_attn_fwd_launches", "lvsa_attn_fwd_grid", "lvsa_workspace_release", "lvsa_schedule_create",
            "lvsa_schedule_num_phases", "lvsa_schedule_index", "lvsa_schedule_attn_fwd", "lvsa_schedule_destroy", "lvsa_last_error", "lvsa_version",
-           "lvsa_build_csr_static")
+           "lvsa_build_csr_static", "lvsa_index_build_launches")
 
 _lib = None
 
@@ -87,6 +87,8 @@ def lib() -> C.CDLL:
         L.lvsa_attn_fwd_grid.argtypes = [C.c_void_p]
         L.lvsa_attn_fwd_launches.restype = C.c_int
         L.lvsa_attn_fwd_launches.argtypes = [C.c_void_p]
+        L.lvsa_index_build_launches.restype = C.c_int
+        L.lvsa_index_build_launches.argtypes = [C.c_void_p]
         L.lvsa_workspace_release.restype = None
         L.lvsa_workspace_release.argtypes = []
         L.lvsa_schedule_create.restype = C.c_int
@@ -176,6 +178,10 @@ class BlockIndex:
 
     def launches(self) -> int:
         return int(lib().lvsa_attn_fwd_launches(self.handle))
+
+    def build_launches(self) -> int:
+        """Kernels the build of this index enqueued (4, or 7 with the quad work lists)."""
+        return int(lib().lvsa_index_build_launches(self.handle))
 
     def destroy(self):
         if self._h:

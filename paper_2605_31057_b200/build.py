@@ -28,23 +28,37 @@ def stale() -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    override = os.environ.get("LVSA_LIB")   # a prebuilt liblvsa.so (e.g. a tuning variant)
-    if override and not force:
-        return override
-    if not force and not stale():
-        return LIB
-    nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    cmd = [nvcc, *NVCC_FLAGS, "-I", INCLUDE, "-I", CSRC, "-o", LIB, *sources()]
+NVCC = "/usr/local/cuda/bin/nvcc"
+
+
+def _compile(out: str, extra_flags=(), verbose: bool = False):
+    cmd = [NVCC, *NVCC_FLAGS, *extra_flags, "-I", INCLUDE, "-I", CSRC, "-o", out, *sources()]
     r = subprocess.run(cmd, capture_output=True, text=True)
     if verbose or r.returncode != 0:
         print(r.stdout)
         print(r.stderr)
     if r.returncode != 0:
-        raise RuntimeError("nvcc failed building liblvsa.so (see output above)")
+        raise RuntimeError("nvcc failed building %s (see output above)" % os.path.basename(out))
+    return cmd, r
+
+
+def build(force: bool = False, verbose: bool = False) -> str:
+    """The product library, rebuilt when a source is newer.  Always this path: nothing outside the call can substitute another library."""
+    if not force and not stale():
+        return LIB
+    cmd, r = _compile(LIB, verbose=verbose)
     with open(os.path.join(CSRC, "build.log"), "w") as f:
         f.write(" ".join(cmd) + "\n" + r.stdout + r.stderr)
     return LIB
+
+
+def build_variant(out: str, extra_flags) -> str:
+    """A separate build of the same sources with extra nvcc flags, written to `out` (never the product
+    path): the fault-injection test compiles one with -DLVSA_TEST_CAP_SHRINK (tests/test_gpu_overflow.py)."""
+    if os.path.abspath(out) == os.path.abspath(LIB):
+        raise ValueError("a variant build must not overwrite the product library")
+    _compile(out, extra_flags=tuple(extra_flags))
+    return out
 
 
 if __name__ == "__main__":

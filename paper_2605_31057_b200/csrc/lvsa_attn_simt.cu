@@ -40,6 +40,8 @@ lvsa_attn_simt_kernel(const T *__restrict__ q, const T *__restrict__ k, const T 
     float *Vs = Ks + BT * KS;           // [BT][D]
     const int i = blockIdx.x, h = blockIdx.y, b = blockIdx.z;
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    // an index whose build overflowed its allocation bound has unfilled lists and a poisoned end (lvsa_index.cu)
+    if (tid == 0 && indptr[gridDim.x] < 0) __trap();
     const long long row0 = (long long)i * BT;
     const size_t tok_stride = (size_t)sn;                                  // token / head / batch strides:
     const size_t base_off = (size_t)b * (size_t)sb + (size_t)h * (size_t)sh;  // lvsa_params_t.layout

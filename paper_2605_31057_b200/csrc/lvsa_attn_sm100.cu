@@ -66,6 +66,8 @@ lvsa_attn_sm100_v0_kernel(const __grid_constant__ CUtensorMap tmap_q,
 
     const int item = blockIdx.x, h = blockIdx.y, b = blockIdx.z;
     const int tid = threadIdx.x, warp = tid >> 5, wg = tid >> 7, rw = tid & 127;
+    // an index whose build overflowed its allocation bound has unfilled lists and a poisoned end (lvsa_index.cu)
+    if (tid == 0 && item_ptr[gridDim.x] < 0) __trap();
 
     if (warp == 0) tmem_alloc<C::TMEM_COLS>(tmem_slot);
     if (tid == 32) {

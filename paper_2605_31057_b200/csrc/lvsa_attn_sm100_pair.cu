@@ -1,8 +1,8 @@
 // CTA-pair LVSA attention forward for sm_100a (d = 128, 128 x 128 tiles): one cluster of two CTAs
 // per work item (pair of adjacent q tiles), tcgen05.mma.cta_group::2 with M = 256 across the pair.
 //
-// Computes Eq. 2 over the kept kv tiles listed by the block index, like
-// lvsa_attn_sm100_ws.cu; what changes is where the operands and accumulators live:
+// Computes Eq. 2 over the kept kv tiles listed by the block index, like the
+// one-CTA-per-item kernel (lvsa_attn_sm100.cu); what changes is where the operands and accumulators live:
 //   * CTA r of the pair owns q tile r of the item: its 128 rows of Q (shared memory), of S / P and
 //     of O (its own TMEM).  Every MMA is one instruction for both CTAs, issued by the leader (CTA 0).
 //   * B operands are split over the pair: CTA r loads kv rows [64 r, 64 r + 64) of K_j (the N
@@ -108,6 +108,8 @@ lvsa_attn_sm100_pair_kernel(const __grid_constant__ CUtensorMap tmap_q,
     extern __shared__ __align__(1024) uint8_t smem_raw[];
     const uint32_t base = smem_u32(smem_raw);
     if ((base & 1023u) != 0u) __trap();   // SWIZZLE_128B tiles and UMMA descriptors need 1024 B
+    // an index whose build overflowed its allocation bound has unfilled lists and a poisoned end (lvsa_index.cu)
+    if (threadIdx.x == 0 && item_ptr[n_items] < 0) __trap();
     uint8_t *base_gen = smem_raw;
     const uint32_t sQ = base + SM::Q_OFF, sRing = base + SM::RING_OFF, sBar = base + SM::BAR_OFF;
     const uint32_t sOut = base + SM::OUT_OFF;
@@ -594,9 +596,25 @@ lvsa_status_t lvsa_make_tmap_bf16(CUtensorMap *m, const void *base, const lvsa_i
 // to the process); `device` must be the current device.
 static int g_pair_n_sm[LVSA_MAX_DEVICES] = {};
 static int g_quad_clusters[LVSA_MAX_DEVICES] = {};   // 4-CTA clusters that can be resident at once
+// HYBRID's internal stream and fork/join events: created here, per device, so that no launch ever
+// creates a resource (a first HYBRID call may already be under stream capture).  `join` is created
+// last and is the "ready" mark: a set-up that failed half-way is retried, not used.
+struct HybridSide { cudaStream_t side = nullptr; cudaEvent_t fork = nullptr, join = nullptr; };
+static HybridSide g_hybrid[LVSA_MAX_DEVICES];
+static std::mutex g_hybrid_mutex;
+static std::mutex g_prepare_mutex;
 lvsa_status_t lvsa_attn_sm100_pair_prepare(int device) {
     if (device < 0 || device >= LVSA_MAX_DEVICES) { lvsa_set_error("device ordinal out of range"); return LVSA_EUNSUPPORTED; }
+    std::lock_guard<std::mutex> prepare_lock(g_prepare_mutex);
     if (g_pair_n_sm[device] != 0) return LVSA_OK;
+    {
+        HybridSide &hs = g_hybrid[device];
+        if (hs.join == nullptr) {
+            if (hs.side == nullptr) LVSA_CUDA_TRY(cudaStreamCreateWithFlags(&hs.side, cudaStreamNonBlocking));
+            if (hs.fork == nullptr) LVSA_CUDA_TRY(cudaEventCreateWithFlags(&hs.fork, cudaEventDisableTiming));
+            LVSA_CUDA_TRY(cudaEventCreateWithFlags(&hs.join, cudaEventDisableTiming));
+        }
+    }
     using SM = SmemP<LVSA_PAIR_STAGES>;
     LVSA_CUDA_TRY(cudaFuncSetAttribute(lvsa_attn_sm100_pair_kernel<LVSA_PAIR_STAGES, MODE_TOKEN0>,
                                        cudaFuncAttributeMaxDynamicSharedMemorySize, SM::BYTES));
@@ -628,14 +646,35 @@ lvsa_status_t lvsa_attn_sm100_pair_prepare(int device) {
 // as two launches that run side by side (the second on an internal stream, forked from and joined back to
 // the caller's stream with events, which also works under stream capture).  The work is split statically
 // at a quad boundary in proportion to the SMs of the two parts.
-struct HybridSide { cudaStream_t side = nullptr; cudaEvent_t fork = nullptr, join = nullptr; };
-static HybridSide g_hybrid[LVSA_MAX_DEVICES];
-static std::mutex g_hybrid_mutex;
 #ifndef LVSA_HYBRID_QUAD_SPEED
 #define LVSA_HYBRID_QUAD_SPEED 1.04   // measured: work per SM and second of the 4-CTA clusters relative to the pairs
 #endif
 
 static bool is_quad(const lvsa_index *ix) { return ix->p.kernel == LVSA_KERNEL_TCGEN05_QUAD || ix->p.kernel == LVSA_KERNEL_TCGEN05_HYBRID; }
+
+// HYBRID's static split over hc heads: quads [0, wq1) go to the 4-CTA clusters, items [item0, item_works) to
+// the CTA pairs on the SMs the clusters cannot cover.  Returns false when everything goes to the clusters
+// (one launch, no fork).
+struct HybridSplit { long long wq1, item0, nqc, pairs_left; };
+static bool hybrid_split(const lvsa_index *ix, int hc, HybridSplit *sp) {
+    const int dev = ix->device;
+    const long long item_works = ix->n_items * hc * ix->p.B, quad_works = ix->n_quads * hc * ix->p.B;
+    sp->nqc = g_quad_clusters[dev]; sp->pairs_left = (g_pair_n_sm[dev] - 4 * sp->nqc) / 2;
+    // the pairs' share of the quads, rounded to whole quads; the pair launch starts at the first item of quad wq1
+    const double share = sp->pairs_left <= 0 ? 0.0 : 2.0 * sp->pairs_left / (4.0 * sp->nqc * LVSA_HYBRID_QUAD_SPEED + 2.0 * sp->pairs_left);
+    sp->wq1 = quad_works - (long long)(quad_works * share + 0.5);
+    if (sp->wq1 < 0) sp->wq1 = 0;
+    sp->item0 = (sp->wq1 / ix->n_quads) * ix->n_items + 2 * (sp->wq1 % ix->n_quads);
+    return !(sp->wq1 == quad_works || sp->item0 >= item_works);
+}
+
+// kernels one launch_heads call over hc heads enqueues (after prepare)
+int lvsa_attn_sm100_pair_num_launches(const lvsa_index *ix, int hc) {
+    if (ix->p.kernel != LVSA_KERNEL_TCGEN05_HYBRID) return 1;
+    HybridSplit sp;
+    if (!hybrid_split(ix, hc, &sp)) return 1;
+    return sp.wq1 > 0 ? 2 : 1;
+}
 
 int lvsa_attn_sm100_pair_grid(const lvsa_index *ix, int hc) {
     if (ix->p.kernel == LVSA_KERNEL_TCGEN05_HYBRID) return g_pair_n_sm[ix->device] / 2 * 2;   // both parts together
@@ -675,22 +714,14 @@ lvsa_status_t lvsa_attn_sm100_pair_launch_heads(const lvsa_index *ix, const void
     const int dev = ix->device;
     const long long item_works = ix->n_items * hc * ix->p.B, quad_works = ix->n_quads * hc * ix->p.B;
     if (ix->p.kernel == LVSA_KERNEL_TCGEN05_HYBRID) {
-        const long long nqc = g_quad_clusters[dev], pairs_left = (g_pair_n_sm[dev] - 4 * nqc) / 2;
-        // the pairs' share of the quads, rounded to whole quads; the pair launch starts at the first item of quad wq1
-        const double share = pairs_left <= 0 ? 0.0 : 2.0 * pairs_left / (4.0 * nqc * LVSA_HYBRID_QUAD_SPEED + 2.0 * pairs_left);
-        long long wq1 = quad_works - (long long)(quad_works * share + 0.5);
-        if (wq1 < 0) wq1 = 0;
-        const long long item0 = (wq1 / ix->n_quads) * ix->n_items + 2 * (wq1 % ix->n_quads);
-        if (wq1 == quad_works || item0 >= item_works) {
+        HybridSplit sp;
+        const bool forks = hybrid_split(ix, hc, &sp);
+        const long long nqc = sp.nqc, pairs_left = sp.pairs_left, wq1 = sp.wq1, item0 = sp.item0;
+        if (!forks) {
             launch(MODE_QUAD, 0, quad_works, nqc, stream);
         } else {
             std::lock_guard<std::mutex> lock(g_hybrid_mutex);
-            HybridSide &hs = g_hybrid[dev];
-            if (hs.side == nullptr) {
-                LVSA_CUDA_TRY(cudaStreamCreateWithFlags(&hs.side, cudaStreamNonBlocking));
-                LVSA_CUDA_TRY(cudaEventCreateWithFlags(&hs.fork, cudaEventDisableTiming));
-                LVSA_CUDA_TRY(cudaEventCreateWithFlags(&hs.join, cudaEventDisableTiming));
-            }
+            HybridSide &hs = g_hybrid[dev];   // created by lvsa_attn_sm100_pair_prepare (above)
             LVSA_CUDA_TRY(cudaEventRecord(hs.fork, stream));
             LVSA_CUDA_TRY(cudaStreamWaitEvent(hs.side, hs.fork, 0));
             launch(MODE_QUAD, 0, wq1, nqc, stream);                      // first: the clusters need whole GPC quarters

@@ -72,7 +72,9 @@ extern "C" {
 const char *lvsa_last_error(void) { return g_last_error.c_str(); }
 
 const char *lvsa_version(void) {
-    return "liblvsa 0.2 (sm_100a; kernels: index-builder, attn-simt-fp32, attn-tcgen05-bf16 (CTA-pair cta_group::2; one-CTA v0))";
+    return "liblvsa 0.3 (sm_100a; kernels: index-builder (handle-based; static-scratch CSR), attn-simt-fp32, "
+           "attn-tcgen05-bf16 (CTA-pair cta_group::2: token-0 and frame-aligned kv tiles; 4-CTA-cluster multicast quad; "
+           "hybrid quad+pair; one-CTA v0))";
 }
 
 lvsa_status_t lvsa_build_block_index_ex(const lvsa_params_t *params, void *stream, lvsa_index_t **out) {
@@ -176,6 +178,10 @@ lvsa_status_t lvsa_attn_fwd(const void *q, const void *k, const void *v, const l
     if ((uintptr_t)lse & 3u) { lvsa_set_error("lse must be 4-byte aligned"); return LVSA_EINVAL; }
     lvsa_status_t dst = check_device(index);
     if (dst != LVSA_OK) return dst;
+    if (index->overflowed) {   // known from an earlier lvsa_index_info / copy_host; unknown yet: the kernel traps
+        lvsa_set_error("internal: the index build exceeded its allocation bound; the index is unusable");
+        return LVSA_ECUDA;
+    }
     index_touch_stream(index, (cudaStream_t)stream);   // the arena is stream-ordered memory
     if (use_tcgen05(index)) return lvsa_attn_sm100_launch(index, q, k, v, out, lse, (cudaStream_t)stream);
     return lvsa_attn_simt_launch(index, q, k, v, out, lse, (cudaStream_t)stream);
@@ -195,6 +201,19 @@ static lvsa_status_t host_pipeline(lvsa_index *ix, HostPipe &hp, int G, const vo
     const size_t pitch = hnd ? (size_t)H * ix->N * ix->p.d * es : (size_t)H * ix->p.d * es;
     const size_t rows = hnd ? (size_t)ix->p.B : (size_t)ix->p.B * ix->N;
     const size_t per_head = hnd ? (size_t)ix->N * ix->p.d * es : (size_t)ix->p.d * es;
+    size_t width_cur = 0;   // bytes per row of the head group being copied (set in the loops below)
+    // HND: the group is B contiguous runs, copied one by one (a 2-D copy would need the batch stride as its
+    // pitch, and cudaMemcpy2D refuses pitches above cudaDevAttrMaxPitch = 2^31 - 1 bytes: H*N*d*2 exceeds
+    // that from about 8.4 M token-heads).  NHD: one 2-D copy, pitch = H*d elements.
+    auto copy_group = [&](uint8_t *dst, const uint8_t *src, cudaMemcpyKind kind, cudaStream_t s) -> lvsa_status_t {
+        if (!hnd) {
+            LVSA_CUDA_TRY(cudaMemcpy2DAsync(dst, pitch, src, pitch, width_cur, rows, kind, s));
+            return LVSA_OK;
+        }
+        for (size_t b = 0; b < rows; ++b)
+            LVSA_CUDA_TRY(cudaMemcpyAsync(dst + b * pitch, src + b * pitch, width_cur, kind, s));
+        return LVSA_OK;
+    };
     // copies start after whatever the caller already enqueued on `stream`
     LVSA_CUDA_TRY(cudaEventRecord(hp.ev_edge, stream));
     LVSA_CUDA_TRY(cudaStreamWaitEvent(hp.s_in, hp.ev_edge, 0));
@@ -202,25 +221,28 @@ static lvsa_status_t host_pipeline(lvsa_index *ix, HostPipe &hp, int G, const vo
     int ng = 0;
     for (int h0 = 0; h0 < H; h0 += per, ++ng) {
         const int hc = h0 + per <= H ? per : H - h0;
-        const size_t off = (size_t)h0 * per_head, width = (size_t)hc * per_head;
+        const size_t off = (size_t)h0 * per_head;
+        width_cur = (size_t)hc * per_head;
         const void *src[3] = {qh, kh, vh};
         void *dst[3] = {s_q, s_k, s_v};
-        for (int t = 0; t < 3; ++t)
-            LVSA_CUDA_TRY(cudaMemcpy2DAsync((uint8_t *)dst[t] + off, pitch, (const uint8_t *)src[t] + off, pitch, width,
-                                            rows, cudaMemcpyHostToDevice, hp.s_in));
+        for (int t = 0; t < 3; ++t) {
+            lvsa_status_t cst = copy_group((uint8_t *)dst[t] + off, (const uint8_t *)src[t] + off, cudaMemcpyHostToDevice, hp.s_in);
+            if (cst != LVSA_OK) return cst;
+        }
         LVSA_CUDA_TRY(cudaEventRecord(hp.ev_in[ng], hp.s_in));
     }
     ng = 0;
     for (int h0 = 0; h0 < H; h0 += per, ++ng) {
         const int hc = h0 + per <= H ? per : H - h0;
-        const size_t off = (size_t)h0 * per_head, width = (size_t)hc * per_head;
+        const size_t off = (size_t)h0 * per_head;
+        width_cur = (size_t)hc * per_head;
         LVSA_CUDA_TRY(cudaStreamWaitEvent(stream, hp.ev_in[ng], 0));
         lvsa_status_t st = lvsa_attn_sm100_pair_launch_heads(ix, s_q, s_k, s_v, s_o, s_lse, h0, hc, stream);
         if (st != LVSA_OK) return st;
         LVSA_CUDA_TRY(cudaEventRecord(hp.ev_c[ng], stream));
         LVSA_CUDA_TRY(cudaStreamWaitEvent(hp.s_out, hp.ev_c[ng], 0));
-        LVSA_CUDA_TRY(cudaMemcpy2DAsync((uint8_t *)oh + off, pitch, (const uint8_t *)s_o + off, pitch, width, rows,
-                                        cudaMemcpyDeviceToHost, hp.s_out));
+        lvsa_status_t cst = copy_group((uint8_t *)oh + off, (const uint8_t *)s_o + off, cudaMemcpyDeviceToHost, hp.s_out);
+        if (cst != LVSA_OK) return cst;
         if (lseh != nullptr)   // lse is [B, H, N]: heads h0.. of every batch are contiguous runs of hc * N floats
             LVSA_CUDA_TRY(cudaMemcpy2DAsync(lseh + (size_t)h0 * ix->N, sizeof(float) * (size_t)H * ix->N,
                                             s_lse + (size_t)h0 * ix->N, sizeof(float) * (size_t)H * ix->N,
@@ -316,6 +338,16 @@ void lvsa_workspace_release(void) {
         cudaSetDevice(dev);
         cudaFree(g_ws[dev].ptr);
         g_ws[dev].ptr = nullptr; g_ws[dev].cap = 0;
+        // the streams and events of the pipelined host path go with the workspace (re-created on demand)
+        HostPipe &hp = g_host[dev];
+        if (hp.s_in != nullptr) cudaStreamDestroy(hp.s_in);
+        if (hp.s_out != nullptr) cudaStreamDestroy(hp.s_out);
+        for (int i = 0; i < HostPipe::MAXG; ++i) {
+            if (hp.ev_in[i] != nullptr) cudaEventDestroy(hp.ev_in[i]);
+            if (hp.ev_c[i] != nullptr) cudaEventDestroy(hp.ev_c[i]);
+        }
+        if (hp.ev_edge != nullptr) cudaEventDestroy(hp.ev_edge);
+        hp = HostPipe();
     }
     if (cur >= 0) cudaSetDevice(cur);
 }
@@ -323,10 +355,19 @@ void lvsa_workspace_release(void) {
 void lvsa_index_destroy(lvsa_index_t *ix) {
     if (ix == nullptr) return;
     if (ix->arena != nullptr) {
+        // the arena and its streams belong to the index's device: make it current around the free
+        int cur = -1;
+        const bool sw = cudaGetDevice(&cur) == cudaSuccess && cur != ix->device;
+        if (sw) cudaSetDevice(ix->device);
         // stream-ordered free behind the work that used the index; if several streams used it,
         // wait for the device first
         if (ix->multi_stream) cudaDeviceSynchronize();
-        cudaFreeAsync(ix->arena, ix->last_stream);
+        if (cudaFreeAsync(ix->arena, ix->last_stream) != cudaSuccess) {
+            cudaGetLastError();                 // e.g. the stream is gone: free synchronously instead
+            cudaDeviceSynchronize();
+            cudaFree(ix->arena);
+        }
+        if (sw) cudaSetDevice(cur);
     }
     delete ix;
 }
@@ -334,6 +375,10 @@ void lvsa_index_destroy(lvsa_index_t *ix) {
 lvsa_status_t lvsa_index_info(const lvsa_index_t *ix, lvsa_index_info_t *info) {
     if (ix == nullptr || info == nullptr) { lvsa_set_error("NULL argument"); return LVSA_EINVAL; }
     memset(info, 0, sizeof(*info));
+    if (!ix->meta_fetched) {   // the counters still have to come from the index's device
+        lvsa_status_t dst = check_device(ix);
+        if (dst != LVSA_OK) return dst;
+    }
     lvsa_status_t fst = lvsa_index_fetch_meta(ix);
     if (fst != LVSA_OK) return fst;
     const lvsa_params_t &p = ix->p;
@@ -355,6 +400,8 @@ lvsa_status_t lvsa_index_copy_host(const lvsa_index_t *ix, int32_t *indptr, int3
                                    uint8_t *flags, int32_t *w_lo, int32_t *w_hi, uint32_t *a_bits) {
     if (ix == nullptr) { lvsa_set_error("NULL index"); return LVSA_EINVAL; }
     const int T = ix->p.T;
+    lvsa_status_t dst = check_device(ix);
+    if (dst != LVSA_OK) return dst;
     lvsa_status_t fst = lvsa_index_fetch_meta(ix);
     if (fst != LVSA_OK) return fst;
     if (indptr) LVSA_CUDA_TRY(cudaMemcpy(indptr, ix->d_indptr, sizeof(int32_t) * ((size_t)ix->nq + 1), cudaMemcpyDeviceToHost));
@@ -430,7 +477,19 @@ void lvsa_schedule_destroy(lvsa_schedule_t *sc) {
     delete sc;
 }
 
-int lvsa_attn_fwd_launches(const lvsa_index_t *ix) { return ix == nullptr ? 0 : 1; }
+int lvsa_attn_fwd_launches(const lvsa_index_t *ix) {
+    if (ix == nullptr) return 0;
+    if (ix->p.kernel != LVSA_KERNEL_TCGEN05_HYBRID) return 1;
+    // HYBRID forks into a 4-CTA-cluster launch and a CTA-pair launch when both parts get work
+    if (check_device(ix) != LVSA_OK || lvsa_attn_sm100_pair_prepare(ix->device) != LVSA_OK) return -1;
+    return lvsa_attn_sm100_pair_num_launches(ix, ix->p.H);
+}
+
+int lvsa_index_build_launches(const lvsa_index_t *ix) {
+    if (ix == nullptr) return 0;
+    // frames, count, scan, fill (+ count, scan, fill of the quad lists); lvsa_index.cu
+    return ix->n_quads != 0 ? 7 : 4;
+}
 
 int lvsa_attn_fwd_grid(const lvsa_index_t *ix) {
     if (ix == nullptr) { lvsa_set_error("NULL index"); return -1; }

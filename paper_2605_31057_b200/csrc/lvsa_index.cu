@@ -104,7 +104,7 @@ __global__ void lvsa_frames_kernel(int T, int W, int a, int s, int tie_hi, int k
 template <bool FILL, bool ALIGNED>
 __global__ void lvsa_tiles_kernel(long long N, int P, int Tv, int Tf, int Bq, int Bk, int nq, int nk, int words,
                                   const uint32_t *__restrict__ a_bits,
-                                  const int32_t *__restrict__ indptr, const int32_t *__restrict__ item_ptr,
+                                  int32_t *__restrict__ indptr, int32_t *__restrict__ item_ptr,
                                   int32_t *__restrict__ counts, int32_t *__restrict__ icounts,
                                   int32_t *__restrict__ indices, uint8_t *__restrict__ flags,
                                   int32_t *__restrict__ item_tiles, int32_t *__restrict__ item_col0,
@@ -112,7 +112,13 @@ __global__ void lvsa_tiles_kernel(long long N, int P, int Tv, int Tf, int Bq, in
     __shared__ int warp_tot[3][32];
     const int g = blockIdx.x, tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int nwarps = blockDim.x >> 5;
-    if (FILL && meta[7]) return;   // allocation bound exceeded (reported by the host)
+    if (FILL && meta[7]) {
+        // Allocation bound exceeded: nothing is filled.  The host reports it at lvsa_index_info /
+        // copy_host; a kernel that is launched on this index anyway must not walk the unfilled lists, so
+        // the list ends are poisoned (negative totals) and the attention kernels trap on them.
+        if (g == 0 && tid == 0) { indptr[nq] = -1; item_ptr[gridDim.x] = -1; }
+        return;
+    }
     // rows and frames of the two q tiles; frame of a token: n / P, tokens past the video (text,
     // R23) belong to the last frame row Tf-1
     const int i0 = 2 * g, i1 = 2 * g + 1;
@@ -217,13 +223,17 @@ __global__ void lvsa_tiles_kernel(long long N, int P, int Tv, int Tf, int Bq, in
 //   FILL = false: qcounts[u];  FILL = true: quad_tiles at quad_ptr[u].
 template <bool FILL>
 __global__ void lvsa_quads_kernel(long long N, int P, int Tf, int Bq, int Bk, int nq, int nk, int words,
-                                  const uint32_t *__restrict__ a_bits, const int32_t *__restrict__ quad_ptr,
+                                  const uint32_t *__restrict__ a_bits, int32_t *__restrict__ quad_ptr,
                                   int32_t *__restrict__ qcounts, int32_t *__restrict__ quad_tiles,
-                                  const int32_t *__restrict__ meta) {
+                                  const int32_t *__restrict__ meta, int32_t *__restrict__ indptr_end,
+                                  int32_t *__restrict__ item_ptr_end) {
     __shared__ int warp_tot[32];
     const int u = blockIdx.x, tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int nwarps = blockDim.x >> 5;
-    if (FILL && meta[7]) return;
+    if (FILL && meta[7]) {   // as in lvsa_tiles_kernel: poison every list end (the quad scan may be the one that overflowed)
+        if (u == 0 && tid == 0) { quad_ptr[gridDim.x] = -1; *indptr_end = -1; *item_ptr_end = -1; }
+        return;
+    }
     int fa[4], fb[4];
 #pragma unroll
     for (int w = 0; w < 4; ++w) {
@@ -270,8 +280,9 @@ __global__ void lvsa_quads_kernel(long long N, int P, int Tf, int Bq, int Bk, in
 }
 
 // Single-block exclusive scan: out[0..n] from counts[0..n-1]; total also to *total_out.
-// If the total exceeds `cap` (the host's allocation bound) meta[7] is raised and the fill passes
-// write nothing; the host reports it at the next lvsa_index_info / copy_host.
+// If the total exceeds `cap` (the host's allocation bound) meta[7] is raised, the fill passes write
+// nothing and poison the list ends (the attention kernels trap on a poisoned index); the host reports
+// it at the next lvsa_index_info / copy_host and lvsa_attn_fwd then refuses the index.
 __global__ void lvsa_scan_kernel(const int32_t *__restrict__ counts_a, int n_a, int32_t *__restrict__ out_a,
                                  int32_t *__restrict__ total_a, long long cap_a,
                                  const int32_t *__restrict__ counts_b, int n_b, int32_t *__restrict__ out_b,
@@ -344,6 +355,9 @@ lvsa_status_t lvsa_index_build_device(lvsa_index *ix, cudaStream_t stream) {
     const long long text_q = p.n_text > 0 ? (p.n_text - 1) / p.tile_q + 2 : 0;
     ix->cap_nnz = per_q * ix->nq + text_q * ix->nk;
     ix->cap_item_tiles = per_item * ix->n_items + text_q * ix->nk;
+#ifdef LVSA_TEST_CAP_SHRINK   // test-only build (tests/test_gpu_overflow.py): an allocation bound that is too small
+    ix->cap_nnz /= LVSA_TEST_CAP_SHRINK; ix->cap_item_tiles /= LVSA_TEST_CAP_SHRINK;
+#endif
     if (ix->cap_nnz >= (1ll << 31) || ix->cap_item_tiles >= (1ll << 31)) {
         lvsa_set_error("index too large for int32 offsets");
         return LVSA_EUNSUPPORTED;
@@ -419,12 +433,14 @@ lvsa_status_t lvsa_index_build_device(lvsa_index *ix, cudaStream_t stream) {
     if (quads) {
         const int nqd = (int)ix->n_quads;
         lvsa_quads_kernel<false><<<nqd, 256, 0, stream>>>((long long)ix->N, p.P, ix->Tf, p.tile_q, p.tile_k, ix->nq, ix->nk,
-                                                          words, ix->d_abits, nullptr, d_qcounts, nullptr, ix->d_meta);
+                                                          words, ix->d_abits, nullptr, d_qcounts, nullptr, ix->d_meta,
+                                                          nullptr, nullptr);
         // block 0 scans the quad counts (total -> quad_meta[0]); block 1 has nothing to do
         lvsa_scan_kernel<<<2, 1024, 0, stream>>>(d_qcounts, nqd, ix->d_quad_ptr, d_quad_meta, (long long)ix->cap_quad_tiles,
                                                  d_qcounts, 0, d_qcounts + nqd, d_quad_meta + 1, 1ll << 40, ix->d_meta + 7);
         lvsa_quads_kernel<true><<<nqd, 256, 0, stream>>>((long long)ix->N, p.P, ix->Tf, p.tile_q, p.tile_k, ix->nq, ix->nk,
-                                                         words, ix->d_abits, ix->d_quad_ptr, nullptr, ix->d_quad_tiles, ix->d_meta);
+                                                         words, ix->d_abits, ix->d_quad_ptr, nullptr, ix->d_quad_tiles, ix->d_meta,
+                                                         ix->d_indptr + ix->nq, ix->d_item_ptr + n_items);
     }
     LVSA_CUDA_TRY(cudaGetLastError());
     ix->meta_fetched = false;
@@ -441,6 +457,7 @@ lvsa_status_t lvsa_index_fetch_meta(const lvsa_index *ix) {
     LVSA_CUDA_TRY(cudaMemcpyAsync(&kept_cols, ix->d_kept_cols, sizeof(kept_cols), cudaMemcpyDeviceToHost, ix->build_stream));
     LVSA_CUDA_TRY(cudaStreamSynchronize(ix->build_stream));
     if (meta[7] != 0) {
+        ix->overflowed = true;   // lvsa_attn_fwd refuses this index from now on
         lvsa_set_error("internal: kept-tile count exceeds the allocation bound");
         return LVSA_ECUDA;
     }

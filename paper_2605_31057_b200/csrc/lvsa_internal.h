@@ -62,6 +62,7 @@ struct lvsa_index {
     mutable int32_t T_per = 0, phase = 0, n_global = 0;
     mutable int64_t nnz = 0, n_partial = 0;
     mutable bool meta_fetched = false;
+    mutable bool overflowed = false;   // the device raised meta[7]: lists unfilled and poisoned
     int device = 0;
     // one stream-ordered arena holds every device buffer below
     void *arena = nullptr;
@@ -131,6 +132,7 @@ lvsa_status_t lvsa_attn_sm100_pair_launch_heads(const lvsa_index *ix, const void
                                                 cudaStream_t stream);
 lvsa_status_t lvsa_attn_sm100_pair_prepare(int device);
 int lvsa_attn_sm100_pair_grid(const lvsa_index *ix, int hc);   // CTAs of a launch over hc heads (after prepare)
+int lvsa_attn_sm100_pair_num_launches(const lvsa_index *ix, int hc);   // kernels of that launch (after prepare)
 int lvsa_attn_uses_pair_kernel(const lvsa_index *ix);   // lvsa_attn_sm100.cu
 
 // lvsa_capi.cu: one-time kernel setup for the index's kernel (used by the schedule driver)

@@ -43,6 +43,18 @@ def test_header_constants_match_binding():
         if f.endswith((".cu", ".cuh", ".h")):
             assert "getenv" not in open(os.path.join(csrc, f)).read(), f
     assert not hasattr(binding.lib(), "lvsa_debug_set_dump")
+    # ... and none in the Python side that picks the library: build.py / binding.py read no environment
+    pkg = os.path.join(ROOT, "paper_2605_31057_b200")
+    for f in ("build.py", "binding.py", "__init__.py", "inputs.py"):
+        src = open(os.path.join(pkg, f)).read()
+        assert "environ" not in src and "getenv" not in src, f
+    assert binding._build.build() == binding._build.LIB
+
+
+def test_version_names_the_variants_compiled_in():
+    v = binding.lvsa_version()
+    for word in ("static-scratch", "quad", "hybrid", "frame-aligned", "CTA-pair", "simt"):
+        assert word in v, word
 
 
 def test_struct_sizes_match_header():

@@ -102,6 +102,17 @@ def test_grid_and_repeatability_and_host_entry_point():
     ixh = build_index(w, w.steps[0], **KERNELS["hybrid"])
     assert ixh.grid() == sms // 2 * 2                                  # clusters of four + pairs: every SM
     hyb, hyb_lse = gpu_attn(w, ixh, q, k, v)
+    # launch counts the library reports (bench.py's gpu_launches): HYBRID forks into two kernels when both
+    # parts get work (B200: 132 SMs in clusters of four, 16 in pairs); 7 builder kernels with quad lists
+    assert ixp.launches() == 1 and ix.launches() == 1
+    assert ixh.launches() == (2 if ix.grid() < sms // 2 * 2 else 1)
+    assert ixp.build_launches() == 4 and ix.build_launches() == 7 and ixh.build_launches() == 7
+    # ... and HYBRID against the oracle itself, not only against its own graph replay
+    rows_h = inputs.sample_rows(w, n_uniform=192, n_edge=64)
+    ref_h, ref_h_lse = oracle_attn(w, q, k, v, w.steps[0], rows_h)
+    st = compare(hyb, hyb_lse, ref_h, ref_h_lse, rows_h)
+    assert st["nan"] == 0 and st["max_abs"] <= BF16_MAX_ABS and st["mean_abs"] <= BF16_MEAN_ABS, st
+    assert st["lse_max_abs"] <= LSE_MAX_ABS_BF16 and st["rel_l2"] <= 2e-2, st
     # CUDA-graph capture of the two side-by-side launches (fork / join with events on an internal stream)
     g, side, out_g = torch.cuda.CUDAGraph(), torch.cuda.Stream(), torch.zeros_like(q)
     side.wait_stream(torch.cuda.current_stream())
@@ -127,8 +138,10 @@ def test_grid_and_repeatability_and_host_entry_point():
 
 @pytest.mark.slow
 @pytest.mark.parametrize("kname", list(KERNELS))
-@pytest.mark.parametrize("name", ["wan1.3b_6x", "hv1.5_2x"])
+@pytest.mark.parametrize("name", ["wan1.3b_1x", "wan1.3b_6x", "wan14b_6x", "hv1.5_2x"])
 def test_large_configs_sampled_rows(name, kname):
+    """Every shape bench.py / profiles/ report a QUAD or HYBRID time for (the four large BASELINE.json configs):
+    1024 sampled rows, edge rows included, against the oracle at full size."""
     w = inputs.WORKLOADS[name]
     rows = inputs.sample_rows(w, n_uniform=768, n_edge=256)
     run_case(w, w.steps[:1], rows=rows, QUAD=KERNELS[kname])
