@@ -28,7 +28,9 @@ sys.path.insert(0, ROOT)
 from paper_2605_31057_b200 import inputs  # noqa: E402
 
 METRIC = "ms/attention call and effective TFLOPS (% of B200 bf16 peak) vs all-tiles dense"
-UNIT = "TFLOP/s (bf16, computed tiles only)"
+UNIT = "TFLOP/s"   # both arms print this unit; what each arm counts is in the line's "unit_detail"
+UNIT_DETAIL = "bf16 in / fp32 accumulate; FLOPs of the computed tiles only (4 d per computed (row, column) pair)"
+REF_UNIT_DETAIL = "fp64; exact Eq. 2 FLOPs (4 d per attended (row, key) pair)"
 FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
 
 
@@ -107,7 +109,10 @@ def ncu_traffic(workload: str):
         for row in csv.DictReader(f):
             if row["workload"] == workload:
                 pct = row.get("tensor_pipe_active_pct")
-                return int(row["dram_bytes_per_launch"]), row["source"], (float(pct) if pct else None)
+                src = row["source"]
+                if row.get("captured"):      # when and on which commit the capture was taken: a stale row shows
+                    src = "captured " + row["captured"] + "; " + src
+                return int(row["dram_bytes_per_launch"]), src, (float(pct) if pct else None)
     return None, None, None
 
 
@@ -128,7 +133,24 @@ def run_ours(args):
         w = dataclasses.replace(w, W=w.W if args.window is None else args.window,
                                 a=w.a if args.anchors is None else args.anchors)
     pk = peaks()
-    q, k, v = inputs.make_qkv(w, f"cuda:{local}", torch.bfloat16, seed=w.seed + rank)
+    from paper_2605_31057_b200 import replicas
+    shard = args.shard == "heads"
+    H_full = w.H
+    if shard:
+        # strong scaling: heads [h_lo, h_hi) of ONE call (same seed on every rank), H_r heads per rank,
+        # no collective; the sub-tensor is made contiguous once, outside any timing
+        import dataclasses
+        h_lo, h_hi = replicas.head_shard(w.H, world, rank)
+        qf, kf, vf = inputs.make_qkv(w, f"cuda:{local}", torch.bfloat16, seed=w.seed)
+        q, k, v = (x[:, :, h_lo:h_hi, :].contiguous() for x in (qf, kf, vf))
+        del qf, kf, vf
+        w = dataclasses.replace(w, H=h_hi - h_lo)
+    else:
+        q, k, v = inputs.make_qkv(w, f"cuda:{local}", torch.bfloat16, seed=w.seed + rank)
+    layout_kw = {}
+    if args.layout == "hnd":   # [B, H, N, d]: every head's tokens contiguous (lvsa_params_t.layout)
+        q, k, v = (x.transpose(1, 2).contiguous() for x in (q, k, v))
+        layout_kw["layout"] = binding.LAYOUT_HND
     out = torch.empty_like(q)
     lse = torch.empty((w.B, w.H, w.N), device=dev, dtype=torch.float32)
     stream = torch.cuda.current_stream()
@@ -139,6 +161,7 @@ def run_ours(args):
 
     def build(s, **kw):
         kw.setdefault("kernel", kernel_of[args.kernel])
+        kw.update(layout_kw)
         return binding.lvsa_build_block_index_ex(
             stream=stream.cuda_stream, T=w.T, P=w.P, H=w.H, d=w.d, B=w.B, window=w.W, anchors=w.a,
             step=s, layer=w.layers[0] if w.layers else 0, n_text=w.n_text, initial_anchors=w.k0, **kw)
@@ -298,12 +321,12 @@ def run_ours(args):
         torch.cuda.synchronize()
         # warm-up: the first creation grows the stream-ordered pool by T_per arenas (milliseconds)
         binding.lvsa_schedule_create(stream=stream.cuda_stream, T=w.T, P=w.P, H=w.H, d=w.d, B=w.B,
-                                     window=w.W, anchors=w.a).destroy()
+                                     window=w.W, anchors=w.a, **layout_kw).destroy()
         torch.cuda.synchronize()
         c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         c0.record(stream)
         sched = binding.lvsa_schedule_create(stream=stream.cuda_stream, T=w.T, P=w.P, H=w.H, d=w.d, B=w.B,
-                                             window=w.W, anchors=w.a)
+                                             window=w.W, anchors=w.a, **layout_kw)
         c1.record(stream)
         torch.cuda.synchronize()
         phases = sched.num_phases()
@@ -336,15 +359,18 @@ def run_ours(args):
     if rank == 0 and not args.no_dense:
         ixd = binding.lvsa_build_block_index_ex(
             stream=stream.cuda_stream, T=w.T, P=w.P, H=w.H, d=w.d, B=w.B, window=w.W,
-            anchors=binding.ALL_TILES, step=0, layer=0)
+            anchors=binding.ALL_TILES, step=0, layer=0, **layout_kw)
         binding.lvsa_attn_fwd(q, k, v, ixd, out, lse, stream.cuda_stream)
         torch.cuda.synchronize()
-        d0, d1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        d0.record(stream)
-        binding.lvsa_attn_fwd(q, k, v, ixd, out, lse, stream.cuda_stream)
-        d1.record(stream)
+        n_dense = 5
+        dev_ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(n_dense)]
+        for d0, d1 in dev_ev:
+            d0.record(stream)
+            binding.lvsa_attn_fwd(q, k, v, ixd, out, lse, stream.cuda_stream)
+            d1.record(stream)
         torch.cuda.synchronize()
-        dense_ms = d0.elapsed_time(d1)
+        dense_all = sorted(d0.elapsed_time(d1) for d0, d1 in dev_ev)
+        dense_ms = float(np.median(dense_all))
         dense_nnz = ixd.info().nnz
         dense_cols = ixd.info().kept_cols
         ixd.destroy()
@@ -357,7 +383,7 @@ def run_ours(args):
         qh, kh, vh = (x.cpu().pin_memory() for x in (q, k, v))
         oh = torch.empty_like(qh).pin_memory()
         lh = torch.empty((w.B, w.H, w.N), dtype=torch.float32).pin_memory()
-        n_e2e = max(1, min(3, args.steps))
+        n_e2e = max(1, args.steps)          # every one of the K steps, like the device-timed loop
         ixh = build(steps_cycle[0])
         binding.lvsa_attn_fwd_host(qh, kh, vh, ixh, oh, lh, stream.cuda_stream)   # warm-up: allocates the workspace
         ixh.destroy()
@@ -376,16 +402,22 @@ def run_ours(args):
         e2e_ms = h0.elapsed_time(h1) / n_e2e
         bi = 3 * q.numel() * q.element_size()
         bo = out.numel() * out.element_size() + lse.numel() * 4
-        e2e = {"ms": e2e_ms, "flops": fl_e2e / n_e2e, "h2d": bi, "d2h": bo}
+        e2e = {"ms": e2e_ms, "flops": fl_e2e / n_e2e, "h2d": bi, "d2h": bo, "calls": n_e2e}
         del qh, kh, vh, oh, lh
 
     # ---- max over ranks, aggregate
-    from paper_2605_31057_b200 import replicas
     ms_step, kern_ms, e2e_max = replicas.max_over_ranks(
         dist, [total_ms / args.steps, kern_ms, e2e["ms"] if e2e else 0.0], device=dev)
     if e2e:
         e2e["ms"] = e2e_max
-    value = replicas.job_throughput(world, tile_flops / args.steps, ms_step) / 1e12
+    if shard:   # the ranks hold different numbers of heads: sum their work, divide by the slowest
+        job_flops, job_e2e_flops = replicas.sum_over_ranks(
+            dist, [tile_flops / args.steps, e2e["flops"] if e2e else 0.0], device=dev)
+        value = replicas.job_throughput_sharded(job_flops, ms_step) / 1e12
+        e2e_value = replicas.job_throughput_sharded(job_e2e_flops, e2e["ms"]) / 1e12 if e2e else None
+    else:
+        value = replicas.job_throughput(world, tile_flops / args.steps, ms_step) / 1e12
+        e2e_value = replicas.job_throughput(world, e2e["flops"], e2e["ms"]) / 1e12 if e2e else None
 
     # ---- CPU baseline: the oracle as it stands, bounded sample (rank 0, N = 1 only)
     cpu = None
@@ -409,41 +441,49 @@ def run_ours(args):
         traffic, traffic_src, tensor_pct = ncu_traffic(args.workload)
         # the exact Eq. 2 work of the same calls (4 d flop per attended key and query row), from the
         # frame-level pattern the library reports (a_bits): what the computed tiles are an upper bound of
-        ix_e = build(steps_cycle[0])
-        ab = ix_e.copy_host().a_bits
-        ix_e.destroy()
-        Tf = ab.shape[0]
         frame_len = np.array([w.P] * w.T + ([w.n_text] if w.n_text else []), dtype=np.float64)
-        bits = ((ab[:, :, None] >> np.arange(32, dtype=np.uint32)[None, None, :]) & 1).reshape(Tf, -1)[:, :Tf]
-        useful = float((frame_len[:, None] * bits * frame_len[None, :]).sum()) * 4.0 * w.d * w.H * w.B
+        useful_of = {}
+        for s_e in sorted(set(steps_cycle)):
+            ix_e = build(s_e)
+            ab = ix_e.copy_host().a_bits
+            ix_e.destroy()
+            Tf = ab.shape[0]
+            bits = ((ab[:, :, None] >> np.arange(32, dtype=np.uint32)[None, None, :]) & 1).reshape(Tf, -1)[:, :Tf]
+            useful_of[s_e] = float((frame_len[:, None] * bits * frame_len[None, :]).sum()) * 4.0 * w.d * w.H * w.B
+        # the timed steps cycle through steps_cycle: average the exact work over the same steps as kern_flops
+        useful = sum(useful_of[steps_cycle[i % len(steps_cycle)]] for i in range(args.steps)) / args.steps
         line = {
             "metric": METRIC, "value": round(value, 2), "unit": UNIT, "n_gpus": world,
+            "unit_detail": UNIT_DETAIL,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": round(ms_step, 4),
-            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
+            "higher_is_better": True, "scaling": "strong" if shard else "weak", "vs_baseline": None, "dtype": "bf16",
             "data": "synthetic (i.i.d. N(0,1) bf16, seeded Philox; stands in for Wan 2.1 latents)",
-            "config": {"workload": args.workload, "T": w.T, "P": w.P, "N": w.N, "H": w.H, "d": w.d,
+            "config": {"workload": args.workload, "T": w.T, "P": w.P, "N": w.N, "H": H_full, "d": w.d,
                        "B": w.B, "tile": w.tile, "window": w.W, "anchors": w.a,
-                       "steps_cycled": steps_cycle, "nnz_mean": nnz_mean, "kernel": args.kernel,
+                       "steps_cycled": steps_cycle, "nnz_mean": nnz_mean, "kernel": args.kernel, "layout": args.layout,
                        "l2": "inputs (3 x %.0f MB) exceed the 126 MB L2; no flush" % (q.numel() * 2 / 1e6),
-                       "parallelism": "replicas only (one independent call per GPU)" if world > 1 else "1 GPU"},
+                       "parallelism": ("heads of one call sharded over %d GPUs (%d heads on rank 0; no collective)" % (world, w.H)) if shard
+                                      else ("replicas only (one independent call per GPU)" if world > 1 else "1 GPU")},
             "ms_per_attention_call": round(kern_ms, 4),
             "ms_per_attention_call_median": round(kern_median, 4), "ms_per_attention_call_min": round(kern_min, 4),
             "tflops_exact_eq2_work": round(useful / (kern_ms * 1e-3) / 1e12, 1),
-            "computed_over_exact_work": round(tile_flop(cols_of[steps_cycle[0]]) / useful, 4),
+            "computed_over_exact_work": round(kern_flops / useful, 4),
             "index_build_us": round(build_us, 1), "index_build_host_enqueue_us": round(build_host_us, 1),
             "pct_of_peak": {"sustained_kernel_vs_sustained_peak_%.1f" % pk["bf16_tflops_sustained"]: round(100 * achieved / pk["bf16_tflops_sustained"], 2),
                             "burst_kernel_vs_burst_peak_%.1f" % pk["bf16_tflops"]: round(100 * burst_tf / pk["bf16_tflops"], 2),
                             "sustained_kernel_vs_burst_peak": round(100 * achieved / pk["bf16_tflops"], 2),
                             "sustained_kernel_vs_nominal_2250": round(100 * achieved / 2250.0, 2)},
             "all_tiles": None if dense_ms is None else {
-                "ms": round(dense_ms, 3), "nnz": int(dense_nnz),
+                "ms": round(dense_ms, 3), "ms_min": round(dense_all[0], 3), "ms_max": round(dense_all[-1], 3),
+                "launches_timed": len(dense_all), "nnz": int(dense_nnz),
                 "speedup_lvsa_vs_all_tiles": round(dense_ms / kern_ms, 3),
                 "tflops": round(tile_flop(dense_cols) / (dense_ms * 1e-3) / 1e12, 1)},
             "frame_aligned_kv_tiles": fa_line,
             "quad_cluster_multicast": quad_line,
             "schedule": sched_line,
             "roofline": {"bound": "tensor", "achieved": round(achieved, 2), "peak": peak_sus,
-                         "unit": "TFLOP/s", "frac": round(achieved / peak_sus, 4), "traffic": traffic,
+                         "unit": "TFLOP/s", "frac": round(achieved / peak_sus, 4),
+                         "frac_exact_eq2": round(useful / (kern_ms * 1e-3) / 1e12 / peak_sus, 4), "traffic": traffic,
                          "peak_source": pk["_source"] + " bf16 SUSTAINED peak: the kernel is timed inside the "
                                         "long step (event pair around each of the %d launches)" % args.steps,
                          "kernel": "lvsa_attn_sm100_pair_kernel", "flops_per_launch": kern_flops,
@@ -456,8 +496,8 @@ def run_ours(args):
                                    "how": "one launch after a 0.25 s idle gap, min of 5, vs the burst peak"}},
             "cpu_baseline": cpu,
             "e2e": None if e2e is None else {
-                "value": round(replicas.job_throughput(world, e2e["flops"], e2e["ms"]) / 1e12, 3), "unit": UNIT,
-                "ms_per_step": round(e2e["ms"], 3), "h2d_bytes_per_step": e2e["h2d"],
+                "value": round(e2e_value, 3), "unit": UNIT,
+                "ms_per_step": round(e2e["ms"], 3), "calls_timed": e2e["calls"], "h2d_bytes_per_step": e2e["h2d"],
                 "d2h_bytes_per_step": e2e["d2h"]},
             "gpu_launches": launches_per_step * args.steps,
             "clocks": clocks,
@@ -480,7 +520,7 @@ def cpu_baseline(w, q, k, v, step, n_rows, nthreads=0):
     keys = sum(int(p.A[r // w.P].sum()) * w.P for r in rows)
     flops = 4.0 * w.d * w.H * keys
     cores = orc.num_threads() if nthreads == 0 else nthreads
-    return {"value": flops / sec / 1e12, "unit": "TFLOP/s (fp64, exact Eq. 2 flops)", "cores": cores,
+    return {"value": flops / sec / 1e12, "unit": UNIT, "unit_detail": REF_UNIT_DETAIL, "cores": cores,
             "kind": "oracle", "seconds": round(sec, 2),
             "sample": f"{len(rows)} seeded query rows x {w.H} heads of {w.name} at step {step}",
             "extrapolated_ms_per_full_call": round(sec * 1e3 * w.N / len(rows), 1)}
@@ -504,8 +544,9 @@ def run_reference(args):
         fl += last["value"] * 1e12 * last["seconds"]
     sec = time.perf_counter() - t0
     val = fl / sec / 1e12
-    ref_unit = "TFLOP/s (fp64, exact Eq. 2 flops)"
-    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": ref_unit, "n_gpus": args.gpus,
+    ref_unit = UNIT
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": ref_unit, "unit_detail": REF_UNIT_DETAIL,
+            "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": sec * 1e3 / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
             "data": "synthetic (same seeded tensors as the CUDA arm)",
@@ -532,6 +573,11 @@ def main():
     ap.add_argument("--no-schedule", action="store_true")
     ap.add_argument("--kernel", default="default", choices=["default", "quad", "hybrid", "v0"],
                     help="attention kernel of the timed steps (default: the CTA-pair kernel); for A/B runs and ncu captures")
+    ap.add_argument("--layout", default="nhd", choices=["nhd", "hnd"],
+                    help="memory order of q, k, v, out: [B,N,H,d] (default, what a QKV projection yields) or [B,H,N,d]")
+    ap.add_argument("--shard", default="none", choices=["none", "heads"],
+                    help="none: every GPU runs a full replica of the call (weak scaling, the default the driver's SCALE run reads); "
+                         "heads: the H heads of ONE call are dealt to the GPUs (strong scaling; PAPER.md:240's Ulysses shards)")
     ap.add_argument("--window", type=int, default=None, help="override W of the workload (sensitivity runs)")
     ap.add_argument("--anchors", type=int, default=None, help="override a = C - (2W+1) of the workload")
     args = ap.parse_args()
