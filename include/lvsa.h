@@ -97,6 +97,14 @@ typedef struct lvsa_params {
     int32_t host_groups;/* lvsa_attn_fwd_host only: number of head groups the call is pipelined over
                            (0 = default: one head per group, at most 16 groups; 1 = unpipelined)      */
     int32_t kv_tiling;  /* LVSA_KV_TILES_TOKEN0 (default) or LVSA_KV_TILES_FRAME_ALIGNED               */
+    /* Free strides (PAPER.md:31 fixes only N = T*P, not where the tokens of q, k, v live).  Per tensor,
+     * the ELEMENT strides of the {token, head, batch} axes; the d elements of one (token, head) are always
+     * contiguous.  An all-zero triplet (the default) means "derive from `layout`".  With them a fused
+     * projection output [B, N, 3, H, d] feeds q, k, v without a copy: pass the three base pointers and
+     * {3*H*d, d, N*3*H*d} for each.  Every stride must be >= 0, a multiple of 16 bytes (8 bf16 / 4 fp32
+     * elements), the token stride >= d, and the byte strides < 2^40 (TMA); else LVSA_EINVAL.  lse stays
+     * [B, H, N].  lvsa_attn_fwd_host takes layout-derived strides only (LVSA_EUNSUPPORTED otherwise). */
+    int64_t stride_q[3], stride_k[3], stride_v[3], stride_out[3];
 } lvsa_params_t;
 
 typedef struct lvsa_index_info {
@@ -211,8 +219,9 @@ lvsa_status_t lvsa_build_csr_static(const lvsa_params_t *params, void *stream, i
  * lvsa_attn_fwd — step a6/a7: Eq. 2 over the kept tiles, exactly (element-level masking on
  * PARTIAL tiles).
  *   q, k, v : DEVICE pointers, contiguous [B, N, H, d] (or [B, H, N, d] when the index was built
- *             with LVSA_LAYOUT_HND), d fastest, bf16 (or fp32 when the index was built with
- *             LVSA_DTYPE_FP32); 16-byte aligned.  Read-only.
+ *             with LVSA_LAYOUT_HND; or with the strides given in lvsa_params_t.stride_q/k/v), d
+ *             fastest, bf16 (or fp32 when the index was built with LVSA_DTYPE_FP32); 16-byte aligned.
+ *             Read-only.
  *   out     : DEVICE pointer, same shape, layout and dtype as q.  Every element is written.
  *   lse     : DEVICE pointer, fp32 [B, H, N], 4-byte aligned, lse = ln sum_{kept} exp(q.k/sqrt d)
  *             (natural log), or NULL.

@@ -41,7 +41,9 @@ class Params(C.Structure):
                                                      ("n_text", C.c_int32),
                                                      ("layout", C.c_int32),
                                                      ("host_groups", C.c_int32),
-                                                     ("kv_tiling", C.c_int32)]
+                                                     ("kv_tiling", C.c_int32),
+                                                     ("stride_q", C.c_int64 * 3), ("stride_k", C.c_int64 * 3),
+                                                     ("stride_v", C.c_int64 * 3), ("stride_out", C.c_int64 * 3)]
 
 
 class IndexInfo(C.Structure):
@@ -238,23 +240,36 @@ def lvsa_build_csr_static(indptr, indices, flags, nnz, stream: int | None = None
                                        _dev_ptr(flags), C.c_int64(cap), _dev_ptr(nnz)))
 
 
-def _dev_ptr(t) -> C.c_void_p:
+def _dev_ptr(t, strided: bool = False) -> C.c_void_p:
     if t is None:
         return C.c_void_p(None)
-    if not t.is_cuda or not t.is_contiguous():
+    if strided:     # a view whose strides the index was built with (lvsa_params_t.stride_*): d must be contiguous
+        if not t.is_cuda or t.stride(-1) != 1:
+            raise ValueError("a strided operand must be a CUDA tensor with a contiguous last axis")
+    elif not t.is_cuda or not t.is_contiguous():
         raise ValueError("lvsa_attn_fwd takes contiguous CUDA tensors")
     return C.c_void_p(t.data_ptr())
 
 
-def lvsa_attn_fwd(q, k, v, index: BlockIndex, out, lse=None, stream: int | None = None):
+def tensor_strides(t):
+    """{token, head, batch} element strides of a [B, N, H, d] view, as lvsa_params_t.stride_q/k/v/out take
+    them (e.g. q = fused[:, :, 0] of a [B, N, 3, H, d] projection output).  The last axis must be contiguous."""
+    if t.dim() != 4 or t.stride(3) != 1:
+        raise ValueError("expected a [B, N, H, d] view with a contiguous last axis")
+    return (t.stride(1), t.stride(2), t.stride(0))
+
+
+def lvsa_attn_fwd(q, k, v, index: BlockIndex, out, lse=None, stream: int | None = None, strided: bool = False):
     """q, k, v, out: CUDA tensors [B, N, H, d] (or [B, H, N, d] for an index built with
     layout=LAYOUT_HND); lse: CUDA fp32 [B, H, N] or None.  Enqueues on
-    `stream` (default: torch's current stream) and returns without synchronising."""
+    `stream` (default: torch's current stream) and returns without synchronising.
+    strided=True: q, k, v, out may be views; the index must have been built with their strides
+    (stride_q=tensor_strides(q), ...), which only the caller can vouch for."""
     if stream is None:
         import torch
         stream = torch.cuda.current_stream().cuda_stream
-    _check(lib().lvsa_attn_fwd(_dev_ptr(q), _dev_ptr(k), _dev_ptr(v), index.handle, _dev_ptr(out),
-                               _dev_ptr(lse), C.c_void_p(stream)))
+    _check(lib().lvsa_attn_fwd(_dev_ptr(q, strided), _dev_ptr(k, strided), _dev_ptr(v, strided), index.handle,
+                               _dev_ptr(out, strided), _dev_ptr(lse), C.c_void_p(stream)))
     return out
 
 

@@ -29,8 +29,8 @@ lvsa_attn_simt_kernel(const T *__restrict__ q, const T *__restrict__ k, const T 
                       T *__restrict__ out, float *__restrict__ lse,
                       const int32_t *__restrict__ indptr, const int32_t *__restrict__ indices,
                       const uint8_t *__restrict__ flags, const uint32_t *__restrict__ a_bits,
-                      int words, long long N, int P, int Tf, int H, long long sn, long long sh, long long sb,
-                      int aligned, int Tv, float scale) {
+                      int words, long long N, int P, int Tf, int H, lvsa_strides sq, lvsa_strides sk, lvsa_strides sv,
+                      lvsa_strides so, int aligned, int Tv, float scale) {
     constexpr int R = BT / SIMT_WARPS;  // rows per warp
     constexpr int CH = D / 32;          // output channels per lane
     constexpr int KS = D + 1;           // padded K row (lane c reads row c: conflict-free)
@@ -43,16 +43,15 @@ lvsa_attn_simt_kernel(const T *__restrict__ q, const T *__restrict__ k, const T 
     // an index whose build overflowed its allocation bound has unfilled lists and a poisoned end (lvsa_index.cu)
     if (tid == 0 && indptr[gridDim.x] < 0) __trap();
     const long long row0 = (long long)i * BT;
-    const size_t tok_stride = (size_t)sn;                                  // token / head / batch strides:
-    const size_t base_off = (size_t)b * (size_t)sb + (size_t)h * (size_t)sh;  // lvsa_params_t.layout
-    const T *qb = q + base_off;
-    const T *kb = k + base_off;
-    const T *vb = v + base_off;
+    // token / head / batch strides per operand: lvsa_params_t.layout or .stride_q/k/v/out
+    const T *qb = q + (size_t)b * (size_t)sq.b + (size_t)h * (size_t)sq.h;
+    const T *kb = k + (size_t)b * (size_t)sk.b + (size_t)h * (size_t)sk.h;
+    const T *vb = v + (size_t)b * (size_t)sv.b + (size_t)h * (size_t)sv.h;
 
     for (int e = tid; e < BT * D; e += blockDim.x) {
         const int r = e / D, c = e % D;
         const long long n = row0 + r;
-        Qs[e] = (n < N) ? to_f32<T>(qb[(size_t)n * tok_stride + c]) : 0.f;
+        Qs[e] = (n < N) ? to_f32<T>(qb[(size_t)n * (size_t)sq.n + c]) : 0.f;
     }
 
     float m[R], l[R], acc[R][CH];
@@ -76,8 +75,8 @@ lvsa_attn_simt_kernel(const T *__restrict__ q, const T *__restrict__ k, const T 
             const int r = x / D, c = x % D;
             const long long n = col0 + r;
             const bool ok = r < kt.width;
-            Ks[r * KS + c] = ok ? to_f32<T>(kb[(size_t)n * tok_stride + c]) : 0.f;
-            Vs[r * D + c] = ok ? to_f32<T>(vb[(size_t)n * tok_stride + c]) : 0.f;
+            Ks[r * KS + c] = ok ? to_f32<T>(kb[(size_t)n * (size_t)sk.n + c]) : 0.f;
+            Vs[r * D + c] = ok ? to_f32<T>(vb[(size_t)n * (size_t)sv.n + c]) : 0.f;
         }
         __syncthreads();
 #pragma unroll
@@ -124,7 +123,7 @@ lvsa_attn_simt_kernel(const T *__restrict__ q, const T *__restrict__ k, const T 
         }
     }
 
-    T *ob = out + base_off;
+    T *ob = out + (size_t)b * (size_t)so.b + (size_t)h * (size_t)so.h;
 #pragma unroll
     for (int r = 0; r < R; ++r) {
         const int rl = wid + r * SIMT_WARPS;
@@ -133,7 +132,7 @@ lvsa_attn_simt_kernel(const T *__restrict__ q, const T *__restrict__ k, const T 
         const float inv = 1.f / l[r];
 #pragma unroll
         for (int c = 0; c < CH; ++c)
-            ob[(size_t)nq * tok_stride + lane + 32 * c] = from_f32<T>(acc[r][c] * inv);
+            ob[(size_t)nq * (size_t)so.n + lane + 32 * c] = from_f32<T>(acc[r][c] * inv);
         if (lse != nullptr && lane == 0)
             lse[((size_t)b * H + h) * N + nq] = m[r] + logf(l[r]);
     }
@@ -146,12 +145,12 @@ lvsa_status_t launch(const lvsa_index *ix, const void *q, const void *k, const v
     auto kern = lvsa_attn_simt_kernel<D, BT, T>;
     LVSA_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const float scale = ix->p.softmax_scale;
-    const lvsa_strides sd = lvsa_layout_strides(ix);
     dim3 grid(ix->nq, ix->p.H, ix->p.B);
     kern<<<grid, SIMT_WARPS * 32, smem, stream>>>(
         (const T *)q, (const T *)k, (const T *)v, (T *)out, lse, ix->d_indptr, ix->d_indices,
-        ix->d_flags, ix->d_abits, ix->words, (long long)ix->N, ix->p.P, ix->Tf, ix->p.H, sd.n, sd.h, sd.b,
-        ix->p.kv_tiling == LVSA_KV_TILES_FRAME_ALIGNED, ix->p.T, scale);
+        ix->d_flags, ix->d_abits, ix->words, (long long)ix->N, ix->p.P, ix->Tf, ix->p.H,
+        lvsa_tensor_strides(ix, LVSA_T_Q), lvsa_tensor_strides(ix, LVSA_T_K), lvsa_tensor_strides(ix, LVSA_T_V),
+        lvsa_tensor_strides(ix, LVSA_T_OUT), ix->p.kv_tiling == LVSA_KV_TILES_FRAME_ALIGNED, ix->p.T, scale);
     LVSA_CUDA_TRY(cudaGetLastError());
     return LVSA_OK;
 }

@@ -288,10 +288,10 @@ PFN_encodeTiled get_encode() {
 // from lvsa_layout_strides (NHD or HND).  Tensor-map dims (fastest first): d, H, N, B whatever the
 // memory order (TMA strides need not be sorted).  Box: 64 x 1 x rows x 1 with SWIZZLE_128B, i.e.
 // smem tile [rows][128 B]; rows >= N are zero-filled.
-lvsa_status_t lvsa_make_tmap_bf16(CUtensorMap *m, const void *base, const lvsa_index *ix, int box_rows) {
+lvsa_status_t lvsa_make_tmap_bf16(CUtensorMap *m, const void *base, const lvsa_index *ix, int box_rows, int which) {
     const long long N = ix->N;
     const int H = ix->p.H, d = ix->p.d, B = ix->p.B;
-    const lvsa_strides sd = lvsa_layout_strides(ix);
+    const lvsa_strides sd = lvsa_tensor_strides(ix, which);   // LVSA_T_Q / K / V / OUT
     PFN_encodeTiled enc = get_encode();
     if (enc == nullptr) { lvsa_set_error("cuTensorMapEncodeTiled entry point not found"); return LVSA_ECUDA; }
     cuuint64_t dims[4] = {(cuuint64_t)d, (cuuint64_t)H, (cuuint64_t)N, (cuuint64_t)B};
@@ -316,9 +316,9 @@ lvsa_status_t launch_v0(const lvsa_index *ix, const void *q, const void *k, cons
     using C = Cfg<D, BT>;
     CUtensorMap mq, mk, mv;
     lvsa_status_t st;
-    if ((st = lvsa_make_tmap_bf16(&mq, q, ix, 128)) != LVSA_OK) return st;
-    if ((st = lvsa_make_tmap_bf16(&mk, k, ix, BT)) != LVSA_OK) return st;
-    if ((st = lvsa_make_tmap_bf16(&mv, v, ix, BT)) != LVSA_OK) return st;
+    if ((st = lvsa_make_tmap_bf16(&mq, q, ix, 128, LVSA_T_Q)) != LVSA_OK) return st;
+    if ((st = lvsa_make_tmap_bf16(&mk, k, ix, BT, LVSA_T_K)) != LVSA_OK) return st;
+    if ((st = lvsa_make_tmap_bf16(&mv, v, ix, BT, LVSA_T_V)) != LVSA_OK) return st;
     auto kern = lvsa_attn_sm100_v0_kernel<D, BT>;
     // the attribute is per device: set once per (instantiation, device)
     static bool ready[LVSA_MAX_DEVICES] = {};
@@ -327,7 +327,7 @@ lvsa_status_t launch_v0(const lvsa_index *ix, const void *q, const void *k, cons
         ready[ix->device] = true;
     }
     const float scale_log2 = ix->p.softmax_scale * 1.4426950408889634f;
-    const lvsa_strides sd = lvsa_layout_strides(ix);
+    const lvsa_strides sd = lvsa_tensor_strides(ix, LVSA_T_OUT);   // the kernel stores `out` with plain stores
     dim3 grid((unsigned)ix->n_items, ix->p.H, ix->p.B);
     kern<<<grid, C::NWG * 128, C::SMEM_BYTES, stream>>>(
         mq, mk, mv, (__nv_bfloat16 *)out, lse, ix->d_item_ptr, ix->d_item_tiles, ix->d_abits, ix->words,

@@ -590,7 +590,7 @@ lvsa_attn_sm100_pair_kernel(const __grid_constant__ CUtensorMap tmap_q,
 }  // namespace
 
 // host side -------------------------------------------------------------------------------
-lvsa_status_t lvsa_make_tmap_bf16(CUtensorMap *m, const void *base, const lvsa_index *ix, int box_rows);
+lvsa_status_t lvsa_make_tmap_bf16(CUtensorMap *m, const void *base, const lvsa_index *ix, int box_rows, int which);
 
 // One-time setup per DEVICE (the shared-memory attribute and the SM count belong to a device, not
 // to the process); `device` must be the current device.
@@ -693,10 +693,10 @@ lvsa_status_t lvsa_attn_sm100_pair_launch_heads(const lvsa_index *ix, const void
     using SM = SmemP<NS>;
     CUtensorMap mq, mk, mv, mo;
     lvsa_status_t st;
-    if ((st = lvsa_make_tmap_bf16(&mq, q, ix, 128)) != LVSA_OK) return st;
-    if ((st = lvsa_make_tmap_bf16(&mk, k, ix, 64)) != LVSA_OK) return st;
-    if ((st = lvsa_make_tmap_bf16(&mv, v, ix, BT)) != LVSA_OK) return st;
-    if ((st = lvsa_make_tmap_bf16(&mo, out, ix, 128)) != LVSA_OK) return st;
+    if ((st = lvsa_make_tmap_bf16(&mq, q, ix, 128, LVSA_T_Q)) != LVSA_OK) return st;
+    if ((st = lvsa_make_tmap_bf16(&mk, k, ix, 64, LVSA_T_K)) != LVSA_OK) return st;
+    if ((st = lvsa_make_tmap_bf16(&mv, v, ix, BT, LVSA_T_V)) != LVSA_OK) return st;
+    if ((st = lvsa_make_tmap_bf16(&mo, out, ix, 128, LVSA_T_OUT)) != LVSA_OK) return st;
     if ((st = lvsa_attn_sm100_pair_prepare(ix->device)) != LVSA_OK) return st;
     const float scale_log2 = ix->p.softmax_scale * 1.4426950408889634f;
     // one launch over the works [work0, work_end) of its kind (quads for MODE_QUAD, items otherwise)

@@ -97,6 +97,24 @@ lvsa_status_t lvsa_build_block_index_ex(const lvsa_params_t *params, void *strea
     if (p.layout != LVSA_LAYOUT_NHD && p.layout != LVSA_LAYOUT_HND) { lvsa_set_error("bad layout"); return LVSA_EINVAL; }
     if (p.host_groups < 0) { lvsa_set_error("host_groups must be >= 0"); return LVSA_EINVAL; }
     if (p.kv_tiling != LVSA_KV_TILES_TOKEN0 && p.kv_tiling != LVSA_KV_TILES_FRAME_ALIGNED) { lvsa_set_error("bad kv_tiling"); return LVSA_EINVAL; }
+    {   // free strides: all-zero triplet = derive from layout; else d contiguous, 16-byte multiples, TMA range
+        const int64_t *st[4] = {p.stride_q, p.stride_k, p.stride_v, p.stride_out};
+        const char *nm[4] = {"stride_q", "stride_k", "stride_v", "stride_out"};
+        const int64_t es = p.dtype == LVSA_DTYPE_FP32 ? 4 : 2;
+        for (int t = 0; t < 4; ++t) {
+            if (!(st[t][0] | st[t][1] | st[t][2])) continue;
+            for (int a = 0; a < 3; ++a) {
+                const int64_t v = st[t][a];
+                if (v < 0 || (v * es) % 16 != 0 || v * es >= (1ll << 40)) {
+                    lvsa_set_error(std::string(nm[t]) + ": strides must be >= 0, multiples of 16 bytes and below 2^40 bytes");
+                    return LVSA_EINVAL;
+                }
+            }
+            if (st[t][0] < p.d) { lvsa_set_error(std::string(nm[t]) + ": the token stride must be >= d (d is contiguous)"); return LVSA_EINVAL; }
+            if (st[t][1] == 0 && p.H > 1) { lvsa_set_error(std::string(nm[t]) + ": the head stride must be > 0 when H > 1"); return LVSA_EINVAL; }
+            if (st[t][2] == 0 && p.B > 1) { lvsa_set_error(std::string(nm[t]) + ": the batch stride must be > 0 when B > 1"); return LVSA_EINVAL; }
+        }
+    }
     if (p.T > 4096) { lvsa_set_error("T > 4096 frames is not supported"); return LVSA_EUNSUPPORTED; }
     if (p.d != 64 && p.d != 128) { lvsa_set_error("head dim must be 64 or 128"); return LVSA_EUNSUPPORTED; }
     if (p.tile_q == 0) p.tile_q = p.d;
@@ -275,6 +293,10 @@ lvsa_status_t lvsa_attn_fwd_host(const void *qh, const void *kh, const void *vh,
     }
     lvsa_status_t dst = check_device(ix);
     if (dst != LVSA_OK) return dst;
+    if (lvsa_has_custom_strides(ix->p)) {
+        lvsa_set_error("lvsa_attn_fwd_host takes layout-derived strides only (stride_q/k/v/out must be zero)");
+        return LVSA_EUNSUPPORTED;
+    }
     cudaStream_t stream = (cudaStream_t)stream_;
     const size_t bytes = (size_t)ix->p.B * ix->N * ix->p.H * ix->p.d * elem_size(ix);
     const size_t lbytes = sizeof(float) * (size_t)ix->p.B * ix->p.H * ix->N;

@@ -100,6 +100,19 @@ inline lvsa_strides lvsa_layout_strides(const lvsa_index *ix) {
     if (ix->p.layout == LVSA_LAYOUT_HND) return {d, N * d, H * N * d};
     return {H * d, d, N * H * d};
 }
+// Strides of one operand: lvsa_params_t.stride_q/k/v/out when given (any non-zero entry), else the layout's.
+enum { LVSA_T_Q = 0, LVSA_T_K = 1, LVSA_T_V = 2, LVSA_T_OUT = 3 };
+inline bool lvsa_has_custom_strides(const lvsa_params_t &p) {
+    const int64_t *t[4] = {p.stride_q, p.stride_k, p.stride_v, p.stride_out};
+    for (int i = 0; i < 4; ++i) if (t[i][0] | t[i][1] | t[i][2]) return true;
+    return false;
+}
+inline lvsa_strides lvsa_tensor_strides(const lvsa_index *ix, int which) {
+    const int64_t *t = which == LVSA_T_Q ? ix->p.stride_q : which == LVSA_T_K ? ix->p.stride_k
+                     : which == LVSA_T_V ? ix->p.stride_v : ix->p.stride_out;
+    if (t[0] | t[1] | t[2]) return {(long long)t[0], (long long)t[1], (long long)t[2]};
+    return lvsa_layout_strides(ix);
+}
 constexpr int LVSA_MAX_DEVICES = 64;   // per-device one-time state is kept in arrays of this size
 
 void lvsa_set_error(const std::string &msg);

@@ -58,8 +58,8 @@ def test_version_names_the_variants_compiled_in():
 
 
 def test_struct_sizes_match_header():
-    # 14 int32 + float + 5 int32; 24 int32 + 6 int64 (include/lvsa.h)
-    assert C.sizeof(binding.Params) == 20 * 4
+    # 14 int32 + float + 5 int32 + 4 x 3 int64; 24 int32 + 6 int64 (include/lvsa.h)
+    assert C.sizeof(binding.Params) == 20 * 4 + 12 * 8 and binding.Params.stride_q.offset == 80
     assert C.sizeof(binding.IndexInfo) == 24 * 4 + 6 * 8
     assert binding.IndexInfo.N.offset == 24 * 4
 
