@@ -53,13 +53,13 @@ class ClockSampler:
          "clocks_event_reasons.sw_power_cap")
 
     def __init__(self, gpu: int):
-        self.gpu, self.rows, self.proc = gpu, [], None
+        self.gpu, self.rows, self.proc, self.first = gpu, [], None, 0
 
     def start(self):
         try:
             self.proc = subprocess.Popen(
                 ["nvidia-smi", "-i", str(self.gpu), f"--query-gpu={self.Q}",
-                 "--format=csv,noheader,nounits", "-lms", "100"],
+                 "--format=csv,noheader,nounits", "-lms", "25"],
                 stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.thr = threading.Thread(target=self._read, daemon=True)
             self.thr.start()
@@ -69,6 +69,10 @@ class ClockSampler:
     def _read(self):
         for line in self.proc.stdout:
             self.rows.append(line.strip())
+
+    def mark(self):
+        """Call at the start of the timed region: stop() then reports only the samples taken after it."""
+        self.first = len(self.rows)
 
     def stop(self):
         if self.proc is None:
@@ -80,7 +84,10 @@ class ClockSampler:
             self.proc.kill()
         sm, mx, reasons = [], [], set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for r in self.rows:
+        rows, window = self.rows[self.first:], "timed region"
+        if not rows and self.rows:      # a region shorter than one sampling period: the sample just before it
+            rows, window = self.rows[-1:], "last sample before the timed region (region shorter than the sampling period)"
+        for r in rows:
             parts = [x.strip() for x in r.split(",")]
             if len(parts) < 6:
                 continue
@@ -93,7 +100,7 @@ class ClockSampler:
                     reasons.add(n)
         return {"sm_mhz": float(np.median(sm)) if sm else None,
                 "sm_max_mhz": max(mx) if mx else None, "reasons": sorted(reasons),
-                "samples": len(sm)}
+                "samples": len(sm), "window": window}
 
 
 def ncu_traffic(workload: str):
@@ -194,18 +201,21 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     # ---- device-resident throughput: K whole steps
-    for i in range(args.warmup):
-        one_step(i)
-    barrier()
+    # nvidia-smi needs a few hundred ms to deliver its first sample: start it before the warm-up and
+    # report only what it saw from the start of the timed region on (sampler.mark below)
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
+    for i in range(args.warmup):
+        one_step(i)
+    barrier()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     # the dominant kernel is timed where it runs: one event pair around the attention launch of
     # every timed step, on the launching stream (events cost nothing on the device)
     ka = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
     kb = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
     barrier()
+    sampler.mark()
     e0.record(stream)
     attn_launches, build_launches = 1, 4
     for i in range(args.steps):
